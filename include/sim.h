@@ -1,0 +1,180 @@
+/*
+ * sim.h -- C ABI of the B200 fast-mode radar raw-data library (libsim.so).
+ *
+ * Method: "fast simulation mode" of Monnier, Camus, Hellouvry, arxiv 2408.11472 (section III).
+ * Every `n_fast` pulses the scene is evaluated once; each illuminated scatterer is summed into a
+ * per-update [range gate x Doppler bin] spectrum (Algorithm 1 + `rasterize`); the
+ * spectra are turned into long-time signals by inverse 1-D DFTs along Doppler and
+ * neighbouring updates are combined with the weights of eq. (1).
+ * The readings taken where the paper is silent are listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - Plain C types only.  Every pointer says whether it is a HOST or a DEVICE pointer.
+ *   - Frame: local Cartesian, z up, flat Earth.  Scatterer arrays are fp32, satellite state fp64.
+ *   - The library never allocates device memory: the caller passes one workspace
+ *     (sim_workspace_bytes) that must outlive the handle.  The library owns only the host handle,
+ *     and (when host staging is enabled) one internal copy stream and a few events.
+ *   - Every call enqueues work on the CUDA stream given to sim_create and returns without
+ *     synchronising, unless stated.  Device inputs must stay valid until the stream reaches that point.
+ *   - Every function returns SIM_OK or a negative SIM_ERR_*; nothing throws, nothing aborts.  After
+ *     an error the handle is unchanged and still usable.  sim_last_error gives a message.
+ *   - Not thread-safe per handle.  Distinct handles are independent.
+ */
+#ifndef PAPER_2408_11472_SIM_H
+#define PAPER_2408_11472_SIM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SIM_OK 0
+#define SIM_ERR_INVALID_ARG (-1) /* NULL pointer, negative count, misaligned array, bad flag */
+#define SIM_ERR_BAD_CONFIG (-2)  /* sizes out of range, N not a power of two, non-positive lambda/PRF/dR */
+#define SIM_ERR_WORKSPACE (-3)   /* workspace too small or not 256-byte aligned */
+#define SIM_ERR_NOT_READY (-4)   /* synthesis needs a spectrum that has not been accumulated */
+#define SIM_ERR_OVERFLOW (-5)    /* more pending spectra than max_pending_updates */
+#define SIM_ERR_CUDA (-6)        /* a CUDA runtime call failed (message in sim_last_error) */
+
+#define SIM_W_SQRT 0   /* eq. (1) of the paper: W = (1 - |i-x|/n_fast)^(1/2); sum of squares = 1 */
+#define SIM_W_LINEAR 1 /* W = 1 - |i-x|/n_fast; partition of unity (reading A1) */
+
+#define SIM_ACC_APPEND 1u /* sim_accumulate_update: add to the current update instead of starting one */
+#define SIM_SYN_FINAL 1u  /* sim_synthesize_pulses: a missing successor spectrum is allowed (tail rule) */
+
+#define SIM_GATE_NONE INT32_MIN /* sim_debug_indices: scatterer touches no gate / is dropped */
+
+typedef struct sim_handle sim_handle; /* opaque, host memory, owned by the library */
+
+typedef struct sim_config {
+  uint32_t struct_size;        /* = sizeof(sim_config); ABI guard */
+  int32_t n_gates;             /* G = n_range of T_fast, 1..1024 */
+  int32_t n_doppler;           /* N = n_doppler of T_fast, power of two, 16..1024 */
+  int32_t pulses_per_update;   /* P = n_fast, >= 1 */
+  int32_t max_pending_updates; /* spectra kept in the ring, >= 2 */
+  int32_t weight_mode;         /* SIM_W_SQRT (default, the paper) or SIM_W_LINEAR */
+  int32_t device;              /* CUDA device ordinal the workspace and stream live on */
+  double wavelength_m;         /* lambda > 0 */
+  double prf_hz;               /* PRF > 0 */
+  double gate_spacing_m;       /* Delta R > 0 */
+  double antenna_alpha;        /* G(theta) = exp(-alpha sin^2 theta) >= 0; 0 = isotropic (reading A10) */
+  int64_t host_stage_scatterers; /* 0, or the H2D chunk size (scatterers) of the *_host entry points */
+  int64_t host_stage_pulses;     /* 0, or the most pulses one sim_synthesize_pulses_host call may ask */
+} sim_config;
+
+/* One batch of scatterers, struct-of-arrays, n entries each (the paper's facets of one tile,
+ * PAPER.md:39).  Pointers are DEVICE pointers for sim_accumulate_update / sim_debug_indices and
+ * HOST pointers (pinned memory for copy/compute overlap) for sim_accumulate_update_host.
+ * Device arrays must be 16-byte aligned.  s0dA = sigma0 * dA (NRCS times facet area, m^2). */
+typedef struct sim_scatterers {
+  const float *x, *y, *z;    /* position, m */
+  const float *vx, *vy, *vz; /* velocity, m/s */
+  const float *s0dA;         /* <= 0 or NaN: the scatterer contributes nothing */
+  uint64_t n;
+} sim_scatterers;
+
+/* Satellite state at the update instant t_u = u * P / PRF; HOST struct, read during
+ * the call. */
+typedef struct sim_sat_state {
+  double pos[3];        /* m */
+  double vel[3];        /* m/s */
+  double boresight[3];  /* antenna axis, any non-zero vector (normalised by the library) */
+  double range_gate0_m; /* range of the centre of gate 0 (reading A9) */
+} sim_sat_state;
+
+typedef struct sim_stats {
+  uint64_t kernel_launches;      /* kernels of this library launched since sim_create */
+  uint64_t updates_accumulated;  /* spectra started */
+  uint64_t scatterers_seen;      /* scatterers passed to sim_accumulate_update[_host] */
+  int64_t pulses_emitted;        /* pulses written by sim_synthesize_pulses[_host] */
+} sim_stats;
+
+/* Bytes of DEVICE workspace sim_create needs for this configuration.  HOST pointers. */
+int sim_workspace_bytes(const sim_config* cfg, size_t* out_bytes);
+
+/* Create a handle.  d_workspace: DEVICE pointer, 256-byte aligned, `bytes` >= sim_workspace_bytes,
+ * owned by the caller and kept alive until sim_destroy.  cuda_stream: a cudaStream_t (NULL = the
+ * legacy default stream).  Initialises the twiddle table on the stream. */
+int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cuda_stream,
+               sim_handle** out);
+
+/* Steps A1-A7: Algorithm 1 body for one surface update.
+ * For every scatterer p: range R = |r_p - r_sat| (scatterers_range), two-gate linear weight from
+ * gf = (R - range_gate0)/dR, Doppler bin k = round(f_D N / PRF) mod N with
+ * f_D = -2 (v_p - v_sat).u / lambda, complex amplitude
+ * sqrt(s0dA) G(theta) / R^2 exp(-i 4 pi R / lambda) (scatterers_complex_amplitudes), summed into the
+ * [G][N] complex64 spectrum of the update (rasterize).
+ * flags = 0: start update u = (number of updates so far), zero its spectrum, accumulate `scat`.
+ * flags = SIM_ACC_APPEND: add another batch (tile) to the update started last.
+ * Errors: SIM_ERR_OVERFLOW when the ring is full of spectra synthesis still needs;
+ * SIM_ERR_INVALID_ARG for NULL / misaligned arrays, APPEND before any update.  scat->n may be 0. */
+int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat,
+                          uint32_t flags);
+
+/* Steps S1-S3: post-processing.  Emits the next n_pulses pulses of the
+ * stream: for pulse x in segment s = floor(x/P),
+ *   Y[x][g] = W_s(x) y_s[g][(x - sP) mod N] + W_{s+1}(x) y_{s+1}[g][(x - (s+1)P) mod N],
+ * y_u = unnormalised inverse DFT of spectrum u along Doppler, W from eq. (1).
+ * d_iq: DEVICE, complex64 [n_pulses][G] (pulse-major, gate fastest, interleaved re/im), 16-byte aligned.
+ * Without SIM_SYN_FINAL every segment touched needs spectra s and s+1 (else SIM_ERR_NOT_READY, nothing
+ * emitted).  With SIM_SYN_FINAL a segment whose successor is absent uses y_s at weight 1.
+ * Spectra older than the segment of the next pulse are released from the ring. */
+int sim_synthesize_pulses(sim_handle* h, int64_t n_pulses, void* d_iq, uint32_t flags);
+
+/* Same two calls with HOST buffers (pinned for overlap): the library stages through the workspace
+ * (cfg.host_stage_scatterers / host_stage_pulses must be > 0) with double-buffered cudaMemcpyAsync.
+ * sim_synthesize_pulses_host enqueues the device-to-host copy on the stream; call sim_synchronize
+ * (or synchronise the stream) before reading h_iq. */
+int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, const sim_sat_state* sat,
+                               uint32_t flags);
+int sim_synthesize_pulses_host(sim_handle* h, int64_t n_pulses, void* h_iq, uint32_t flags);
+
+/* Blocks until all work enqueued by this handle has finished. */
+int sim_synchronize(sim_handle* h);
+
+/* Frees the host handle (and internal stream/events).  NULL-safe.  The workspace stays the caller's. */
+int sim_destroy(sim_handle* h);
+
+/* ---- parity / debug / multi-GPU support ------------------------------------------------------ */
+
+/* Copies spectrum `update_index` (must still be in the ring) to d_out: DEVICE complex64 [G][N],
+ * bin fastest.  Asynchronous on the stream. */
+int sim_get_spectrum(sim_handle* h, int64_t update_index, void* d_out);
+
+/* Byte offset of spectrum `update_index` inside the caller's workspace (so that the caller can
+ * all-reduce partial spectra across GPUs in place). */
+int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset);
+
+/* Runs the production index computation only: for each scatterer the gate g0 = floor(gf) in
+ * [-1, G-1] and the Doppler bin k in [0, N); dropped scatterers give (SIM_GATE_NONE, -1).
+ * d_gate0, d_bin: DEVICE int32[n].  Must match the canonical fp64 sequence bit for bit. */
+int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat,
+                      int32_t* d_gate0, int32_t* d_bin);
+
+/* Tuning knobs (benchmarks and tests; defaults are chosen by the library). */
+#define SIM_OPT_ACC_VARIANT 1   /* 0 = reference kernel (global atomics), 1 = shared-memory tile kernel */
+#define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto */
+#define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit; 0 = auto */
+#define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto */
+#define SIM_OPT_ACC_REPLICAS 5  /* shared-memory replicas of the tile; 0 = auto */
+#define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band */
+int sim_set_option(sim_handle* h, int32_t option, int64_t value);
+
+int sim_get_stats(const sim_handle* h, sim_stats* out);
+
+/* Synchronises the stream, copies the library's device counters to h_out (HOST, 4 x uint32:
+ * [0] scheduling tickets of the last accumulation launch, [1] contributions that missed the
+ * shared-memory window and went to global atomics, [2] tile flushes, [3] reserved) and, when
+ * reset != 0, zeroes them. */
+int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset);
+
+/* Message of the last error on this handle ("" if none); valid until the next call.  h may be NULL
+ * (returns the message of the last failed sim_create / sim_workspace_bytes on this thread). */
+const char* sim_last_error(const sim_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_2408_11472_SIM_H */

@@ -1,0 +1,505 @@
+// Host side of libsim.so: the C ABI of include/sim.h.  Validation, ring bookkeeping, constant
+// derivation in fp64, kernel launches.  No device allocation happens here: everything lives in the
+// caller's workspace.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "sim_internal.h"
+
+using namespace simk;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  size_t ring_off, slot_bytes, tw_off, ctr_off, stage_off, stage_buf_bytes, iq_off, iq_bytes, total;
+};
+
+Layout make_layout(const sim_config& c) {
+  Layout L{};
+  size_t off = 0;
+  L.ring_off = off;
+  L.slot_bytes = align_up((size_t)c.n_gates * c.n_doppler * sizeof(float2), 256);
+  off += L.slot_bytes * (size_t)c.max_pending_updates;
+  L.tw_off = off;
+  off += align_up((size_t)(c.n_doppler / 2) * sizeof(float2), 256);
+  L.ctr_off = off;
+  off += align_up(kNumCounters * sizeof(unsigned int), 256);
+  L.stage_off = off;
+  L.stage_buf_bytes = align_up((size_t)c.host_stage_scatterers * sizeof(float), 256) * 7;
+  off += 2 * L.stage_buf_bytes;
+  L.iq_off = off;
+  L.iq_bytes = align_up((size_t)c.host_stage_pulses * c.n_gates * sizeof(float2), 256);
+  off += L.iq_bytes;
+  L.total = off;
+  return L;
+}
+
+const char* check_config(const sim_config* c) {
+  if (!c) return "cfg is NULL";
+  if (c->struct_size != sizeof(sim_config)) return "cfg.struct_size != sizeof(sim_config) (ABI mismatch)";
+  if (c->n_gates < 1 || c->n_gates > 1024) return "n_gates must be in 1..1024";
+  if (c->n_doppler < 16 || c->n_doppler > 1024 || (c->n_doppler & (c->n_doppler - 1)))
+    return "n_doppler must be a power of two in 16..1024";
+  if (c->pulses_per_update < 1) return "pulses_per_update must be >= 1";
+  if (c->max_pending_updates < 2) return "max_pending_updates must be >= 2";
+  if (c->weight_mode != SIM_W_SQRT && c->weight_mode != SIM_W_LINEAR) return "unknown weight_mode";
+  if (!(c->wavelength_m > 0) || !std::isfinite(c->wavelength_m)) return "wavelength_m must be > 0";
+  if (!(c->prf_hz > 0) || !std::isfinite(c->prf_hz)) return "prf_hz must be > 0";
+  if (!(c->gate_spacing_m > 0) || !std::isfinite(c->gate_spacing_m)) return "gate_spacing_m must be > 0";
+  if (!(c->antenna_alpha >= 0) || !std::isfinite(c->antenna_alpha)) return "antenna_alpha must be >= 0";
+  if (c->host_stage_scatterers < 0 || c->host_stage_pulses < 0) return "host staging sizes must be >= 0";
+  if (c->host_stage_scatterers % 4) return "host_stage_scatterers must be a multiple of 4";
+  if (c->device < 0) return "device must be >= 0";
+  return nullptr;
+}
+
+}  // namespace
+
+struct sim_handle {
+  sim_config cfg;
+  Layout lay;
+  unsigned char* ws;
+  cudaStream_t stream;
+  cudaStream_t copy_stream;      // only with host staging
+  cudaEvent_t ev_copied[2];      // staging buffer b filled
+  cudaEvent_t ev_consumed[2];    // staging buffer b consumed by the kernel
+  bool stage_used[2];
+  int sm_count;
+  size_t smem_optin;
+  // stream state
+  int64_t n_updates;             // spectra started so far
+  int64_t pulses_emitted;
+  // tuning
+  int opt_variant, opt_blocks, opt_window, opt_replicas, opt_index_path;
+  int64_t opt_superchunk;
+  // stats
+  uint64_t launches, scatterers_seen;
+  std::string err;
+};
+
+namespace {
+
+int fail(sim_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return code;
+}
+int cuda_fail(sim_handle* h, cudaError_t e, const char* what) {
+  return fail(h, SIM_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+float2* slot_ptr(sim_handle* h, int64_t u) {
+  return reinterpret_cast<float2*>(h->ws + h->lay.ring_off + (size_t)(u % h->cfg.max_pending_updates) * h->lay.slot_bytes);
+}
+unsigned int* counters(sim_handle* h) { return reinterpret_cast<unsigned int*>(h->ws + h->lay.ctr_off); }
+
+int64_t oldest_needed(const sim_handle* h) { return h->pulses_emitted / h->cfg.pulses_per_update; }
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+int check_scatterers(sim_handle* h, const sim_scatterers* s, bool device_ptrs) {
+  if (!s) return fail(h, SIM_ERR_INVALID_ARG, "scatterers is NULL");
+  if (s->n == 0) return SIM_OK;
+  const float* a[7] = {s->x, s->y, s->z, s->vx, s->vy, s->vz, s->s0dA};
+  for (int i = 0; i < 7; ++i) {
+    if (!a[i]) return fail(h, SIM_ERR_INVALID_ARG, "a scatterer array is NULL");
+    if (device_ptrs && misaligned(a[i])) return fail(h, SIM_ERR_INVALID_ARG, "scatterer arrays must be 16-byte aligned");
+  }
+  return SIM_OK;
+}
+
+int check_sat(sim_handle* h, const sim_sat_state* sat) {
+  if (!sat) return fail(h, SIM_ERR_INVALID_ARG, "sat_state is NULL");
+  const double b2 = sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
+                    sat->boresight[2] * sat->boresight[2];
+  if (!(b2 > 0) || !std::isfinite(b2)) return fail(h, SIM_ERR_INVALID_ARG, "boresight must be a finite non-zero vector");
+  for (int i = 0; i < 3; ++i)
+    if (!std::isfinite(sat->pos[i]) || !std::isfinite(sat->vel[i])) return fail(h, SIM_ERR_INVALID_ARG, "sat_state is not finite");
+  if (!std::isfinite(sat->range_gate0_m)) return fail(h, SIM_ERR_INVALID_ARG, "range_gate0_m is not finite");
+  return SIM_OK;
+}
+
+// Tile geometry: W Doppler bins x G gates x R replicas of float2 in shared memory.
+void choose_tile(const sim_handle* h, int* W, int* R) {
+  const int G = h->cfg.n_gates, N = h->cfg.n_doppler;
+  const size_t budget = h->smem_optin > 64 * 1024 ? h->smem_optin - 16 * 1024 : 32 * 1024;
+  int w = h->opt_window > 0 ? h->opt_window : 16;
+  if (w > N) w = N;
+  int r = h->opt_replicas > 0 ? h->opt_replicas : 8;
+  while (r > 1 && (size_t)G * w * r * sizeof(float2) > budget) r >>= 1;
+  while (w > 1 && (size_t)G * w * r * sizeof(float2) > budget) w >>= 1;
+  *W = w;
+  *R = r;
+}
+
+AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sat, float2* T) {
+  AccParams p{};
+  p.x = s->x; p.y = s->y; p.z = s->z; p.vx = s->vx; p.vy = s->vy; p.vz = s->vz; p.s0dA = s->s0dA;
+  p.n = s->n;
+  p.sx = sat->pos[0]; p.sy = sat->pos[1]; p.sz = sat->pos[2];
+  p.svx = sat->vel[0]; p.svy = sat->vel[1]; p.svz = sat->vel[2];
+  p.rg0 = sat->range_gate0_m;
+  // host constants of the canonical sequence, each by exactly this expression
+  p.inv_dR = 1.0 / h->cfg.gate_spacing_m;
+  p.two_over_lambda = 2.0 / h->cfg.wavelength_m;
+  p.cD = (-2.0 * (double)h->cfg.n_doppler) / (h->cfg.wavelength_m * h->cfg.prf_hz);
+  const double bn = std::sqrt(sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
+                              sat->boresight[2] * sat->boresight[2]);
+  p.bx = (float)(sat->boresight[0] / bn);
+  p.by = (float)(sat->boresight[1] / bn);
+  p.bz = (float)(sat->boresight[2] / bn);
+  p.alpha = (float)h->cfg.antenna_alpha;
+  p.G = h->cfg.n_gates;
+  p.N = h->cfg.n_doppler;
+  p.T = T;
+  p.counters = counters(h);
+  choose_tile(h, &p.W, &p.R);
+  const int blocks = h->opt_blocks > 0 ? h->opt_blocks : h->sm_count;
+  unsigned long long sc = (unsigned long long)h->opt_superchunk;
+  if (sc == 0) {
+    // aim at >= 8 scheduling units per block, between one chunk and 64K scatterers
+    sc = 65536;
+    while (sc > (unsigned long long)kAccChunk && s->n / sc < (unsigned long long)blocks * 8) sc >>= 1;
+  }
+  sc = (sc + kAccChunk - 1) / kAccChunk * kAccChunk;
+  p.superchunk = sc;
+  p.index_path = h->opt_index_path;
+  return p;
+}
+
+int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, float2* T) {
+  AccParams p = make_acc_params(h, d_scat, sat, T);
+  const int blocks = h->opt_blocks > 0 ? h->opt_blocks : h->sm_count;
+  int l = 0;
+  cudaError_t e = launch_accumulate(p, h->opt_variant, blocks, h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
+  return SIM_OK;
+}
+
+// Common front of the two accumulate entry points: validates, opens a new update if asked.
+int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sat, uint32_t flags,
+                 bool device_ptrs, float2** T) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (flags & ~SIM_ACC_APPEND) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulate flag");
+  int rc = check_scatterers(h, s, device_ptrs);
+  if (rc) return rc;
+  rc = check_sat(h, sat);
+  if (rc) return rc;
+  if (flags & SIM_ACC_APPEND) {
+    if (h->n_updates == 0) return fail(h, SIM_ERR_INVALID_ARG, "SIM_ACC_APPEND before any update");
+    *T = slot_ptr(h, h->n_updates - 1);
+    return SIM_OK;
+  }
+  if (h->n_updates - oldest_needed(h) >= h->cfg.max_pending_updates)
+    return fail(h, SIM_ERR_OVERFLOW, "ring full: synthesize pulses before accumulating another update");
+  *T = slot_ptr(h, h->n_updates);
+  cudaError_t e = cudaMemsetAsync(*T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
+  ++h->n_updates;
+  return SIM_OK;
+}
+
+int plan_synthesis(sim_handle* h, int64_t n_pulses, const void* iq, uint32_t flags, int64_t* s_first,
+                   int64_t* s_last) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (flags & ~SIM_SYN_FINAL) return fail(h, SIM_ERR_INVALID_ARG, "unknown synthesize flag");
+  if (n_pulses < 0) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses < 0");
+  if (n_pulses == 0) return SIM_OK;
+  if (!iq) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer is NULL");
+  const int64_t P = h->cfg.pulses_per_update;
+  *s_first = h->pulses_emitted / P;
+  *s_last = (h->pulses_emitted + n_pulses - 1) / P;
+  if (*s_last >= h->n_updates) return fail(h, SIM_ERR_NOT_READY, "spectrum of the last segment has not been accumulated");
+  if (*s_last + 1 >= h->n_updates && !(flags & SIM_SYN_FINAL))
+    return fail(h, SIM_ERR_NOT_READY, "successor spectrum missing (accumulate it or pass SIM_SYN_FINAL)");
+  return SIM_OK;
+}
+
+int do_synthesize(sim_handle* h, int64_t n_pulses, float2* d_iq, int64_t s_first, int64_t s_last) {
+  SynParams p{};
+  p.ring = reinterpret_cast<const float2*>(h->ws + h->lay.ring_off);
+  p.slot_stride = h->lay.slot_bytes / sizeof(float2);
+  p.cap = h->cfg.max_pending_updates;
+  p.tw = reinterpret_cast<const float2*>(h->ws + h->lay.tw_off);
+  p.iq = d_iq;
+  p.x0 = h->pulses_emitted;
+  p.n_pulses = n_pulses;
+  p.seg0 = s_first;
+  p.n_spectra = h->n_updates;
+  p.G = h->cfg.n_gates;
+  p.N = h->cfg.n_doppler;
+  p.logN = 0;
+  while ((1 << p.logN) < p.N) ++p.logN;
+  p.P = h->cfg.pulses_per_update;
+  p.GT = synth_gate_tile(p.N);
+  p.weight_mode = h->cfg.weight_mode;
+  int l = 0;
+  cudaError_t e = launch_synthesize(p, (int)(s_last - s_first + 1), h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) return cuda_fail(h, e, "synthesize launch");
+  h->pulses_emitted += n_pulses;
+  return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sim_workspace_bytes(const sim_config* cfg, size_t* out_bytes) {
+  if (!out_bytes) return fail(nullptr, SIM_ERR_INVALID_ARG, "out_bytes is NULL");
+  if (const char* m = check_config(cfg)) return fail(nullptr, cfg ? SIM_ERR_BAD_CONFIG : SIM_ERR_INVALID_ARG, m);
+  *out_bytes = make_layout(*cfg).total;
+  return SIM_OK;
+}
+
+int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cuda_stream, sim_handle** out) {
+  if (!out) return fail(nullptr, SIM_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (const char* m = check_config(cfg)) return fail(nullptr, cfg ? SIM_ERR_BAD_CONFIG : SIM_ERR_INVALID_ARG, m);
+  const Layout lay = make_layout(*cfg);
+  if (!d_workspace) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace is NULL");
+  if (reinterpret_cast<uintptr_t>(d_workspace) & 255u) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+  if (bytes < lay.total) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace smaller than sim_workspace_bytes");
+  cudaError_t e = cudaSetDevice(cfg->device);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
+  sim_handle* h = new (std::nothrow) sim_handle();
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "out of host memory");
+  h->cfg = *cfg;
+  h->lay = lay;
+  h->ws = static_cast<unsigned char*>(d_workspace);
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  h->copy_stream = nullptr;
+  h->stage_used[0] = h->stage_used[1] = false;
+  h->n_updates = 0;
+  h->pulses_emitted = 0;
+  h->opt_variant = 1;
+  h->opt_blocks = 0;
+  h->opt_window = 0;
+  h->opt_replicas = 0;
+  h->opt_index_path = 0;
+  h->opt_superchunk = 0;
+  h->launches = 0;
+  h->scatterers_seen = 0;
+  int v = 0;
+  e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cfg->device);
+  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)"); }
+  h->sm_count = v;
+  e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
+  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem optin)"); }
+  h->smem_optin = (size_t)v;
+  if (cfg->host_stage_scatterers > 0 || cfg->host_stage_pulses > 0) {
+    e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaStreamCreate(copy)"); }
+    for (int b = 0; b < 2; ++b) {
+      cudaEventCreateWithFlags(&h->ev_copied[b], cudaEventDisableTiming);
+      cudaEventCreateWithFlags(&h->ev_consumed[b], cudaEventDisableTiming);
+    }
+  }
+  e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters)"); }
+  int l = 0;
+  e = launch_twiddles(reinterpret_cast<float2*>(h->ws + lay.tw_off), cfg->n_doppler, h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "twiddle launch"); }
+  *out = h;
+  return SIM_OK;
+}
+
+int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, uint32_t flags) {
+  float2* T = nullptr;
+  int rc = begin_update(h, d_scat, sat, flags, true, &T);
+  if (rc) return rc;
+  h->scatterers_seen += d_scat->n;
+  return do_accumulate(h, d_scat, sat, T);
+}
+
+int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, const sim_sat_state* sat, uint32_t flags) {
+  if (h && h->cfg.host_stage_scatterers <= 0) return fail(h, SIM_ERR_INVALID_ARG, "host staging disabled (cfg.host_stage_scatterers == 0)");
+  float2* T = nullptr;
+  int rc = begin_update(h, h_scat, sat, flags, false, &T);
+  if (rc) return rc;
+  h->scatterers_seen += h_scat->n;
+  const uint64_t chunk = (uint64_t)h->cfg.host_stage_scatterers;
+  const size_t arr_stride = h->lay.stage_buf_bytes / 7;  // bytes between staged arrays
+  const float* src[7] = {h_scat->x, h_scat->y, h_scat->z, h_scat->vx, h_scat->vy, h_scat->vz, h_scat->s0dA};
+  int b = 0;
+  for (uint64_t off = 0; off < h_scat->n; off += chunk, b ^= 1) {
+    const uint64_t m = (h_scat->n - off < chunk) ? h_scat->n - off : chunk;
+    unsigned char* buf = h->ws + h->lay.stage_off + (size_t)b * h->lay.stage_buf_bytes;
+    cudaError_t e;
+    if (h->stage_used[b]) {
+      e = cudaStreamWaitEvent(h->copy_stream, h->ev_consumed[b], 0);  // kernel done with this buffer
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(consumed)");
+    }
+    for (int a = 0; a < 7; ++a) {
+      e = cudaMemcpyAsync(buf + a * arr_stride, src[a] + off, m * sizeof(float), cudaMemcpyHostToDevice, h->copy_stream);
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(H2D scatterers)");
+    }
+    e = cudaEventRecord(h->ev_copied[b], h->copy_stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(copied)");
+    e = cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(copied)");
+    sim_scatterers d{};
+    d.x = reinterpret_cast<const float*>(buf + 0 * arr_stride);
+    d.y = reinterpret_cast<const float*>(buf + 1 * arr_stride);
+    d.z = reinterpret_cast<const float*>(buf + 2 * arr_stride);
+    d.vx = reinterpret_cast<const float*>(buf + 3 * arr_stride);
+    d.vy = reinterpret_cast<const float*>(buf + 4 * arr_stride);
+    d.vz = reinterpret_cast<const float*>(buf + 5 * arr_stride);
+    d.s0dA = reinterpret_cast<const float*>(buf + 6 * arr_stride);
+    d.n = m;
+    rc = do_accumulate(h, &d, sat, T);
+    if (rc) return rc;
+    e = cudaEventRecord(h->ev_consumed[b], h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(consumed)");
+    h->stage_used[b] = true;
+  }
+  return SIM_OK;
+}
+
+int sim_synthesize_pulses(sim_handle* h, int64_t n_pulses, void* d_iq, uint32_t flags) {
+  int64_t s0 = 0, s1 = -1;
+  int rc = plan_synthesis(h, n_pulses, d_iq, flags, &s0, &s1);
+  if (rc || n_pulses == 0) return rc;
+  if (misaligned(d_iq)) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer must be 16-byte aligned");
+  return do_synthesize(h, n_pulses, static_cast<float2*>(d_iq), s0, s1);
+}
+
+int sim_synthesize_pulses_host(sim_handle* h, int64_t n_pulses, void* h_iq, uint32_t flags) {
+  if (h && n_pulses > h->cfg.host_stage_pulses) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses exceeds cfg.host_stage_pulses");
+  int64_t s0 = 0, s1 = -1;
+  int rc = plan_synthesis(h, n_pulses, h_iq, flags, &s0, &s1);
+  if (rc || n_pulses == 0) return rc;
+  float2* d_iq = reinterpret_cast<float2*>(h->ws + h->lay.iq_off);
+  rc = do_synthesize(h, n_pulses, d_iq, s0, s1);
+  if (rc) return rc;
+  cudaError_t e = cudaMemcpyAsync(h_iq, d_iq, (size_t)n_pulses * h->cfg.n_gates * sizeof(float2), cudaMemcpyDeviceToHost, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(D2H iq)");
+  return SIM_OK;
+}
+
+int sim_synchronize(sim_handle* h) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  cudaError_t e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamSynchronize");
+  if (h->copy_stream) {
+    e = cudaStreamSynchronize(h->copy_stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamSynchronize(copy)");
+  }
+  return SIM_OK;
+}
+
+int sim_destroy(sim_handle* h) {
+  if (!h) return SIM_OK;
+  if (h->copy_stream) {
+    cudaStreamSynchronize(h->copy_stream);
+    for (int b = 0; b < 2; ++b) {
+      cudaEventDestroy(h->ev_copied[b]);
+      cudaEventDestroy(h->ev_consumed[b]);
+    }
+    cudaStreamDestroy(h->copy_stream);
+  }
+  delete h;
+  return SIM_OK;
+}
+
+int sim_get_spectrum(sim_handle* h, int64_t update_index, void* d_out) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (!d_out) return fail(h, SIM_ERR_INVALID_ARG, "d_out is NULL");
+  if (update_index < 0 || update_index >= h->n_updates || update_index < h->n_updates - h->cfg.max_pending_updates)
+    return fail(h, SIM_ERR_INVALID_ARG, "spectrum not in the ring");
+  cudaError_t e = cudaMemcpyAsync(d_out, slot_ptr(h, update_index), (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2),
+                                  cudaMemcpyDeviceToDevice, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(spectrum)");
+  return SIM_OK;
+}
+
+int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (!out_offset) return fail(h, SIM_ERR_INVALID_ARG, "out_offset is NULL");
+  if (update_index < 0 || update_index >= h->n_updates || update_index < h->n_updates - h->cfg.max_pending_updates)
+    return fail(h, SIM_ERR_INVALID_ARG, "spectrum not in the ring");
+  *out_offset = (size_t)(reinterpret_cast<unsigned char*>(slot_ptr(h, update_index)) - h->ws);
+  return SIM_OK;
+}
+
+int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, int32_t* d_gate0, int32_t* d_bin) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (!d_scat) return fail(h, SIM_ERR_INVALID_ARG, "scatterers is NULL");
+  if (d_scat->n && (!d_gate0 || !d_bin)) return fail(h, SIM_ERR_INVALID_ARG, "output arrays are NULL");
+  sim_scatterers s = *d_scat;
+  if (!s.s0dA) s.s0dA = s.x;  // not consulted by the index kernel
+  int rc = check_scatterers(h, &s, true);
+  if (rc) return rc;
+  rc = check_sat(h, sat);
+  if (rc) return rc;
+  AccParams p = make_acc_params(h, &s, sat, nullptr);
+  int l = 0;
+  cudaError_t e = launch_indices(p, d_gate0, d_bin, h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
+  return SIM_OK;
+}
+
+int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (value < 0) return fail(h, SIM_ERR_INVALID_ARG, "option value < 0");
+  switch (option) {
+    case SIM_OPT_ACC_VARIANT:
+      if (value > 1) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
+      h->opt_variant = (int)value;
+      return SIM_OK;
+    case SIM_OPT_ACC_BLOCKS:
+      if (value > 65535) return fail(h, SIM_ERR_INVALID_ARG, "too many blocks");
+      h->opt_blocks = (int)value;
+      return SIM_OK;
+    case SIM_OPT_ACC_SUPERCHUNK:
+      h->opt_superchunk = value;
+      return SIM_OK;
+    case SIM_OPT_ACC_WINDOW_BINS:
+      if (value & (value - 1)) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two");
+      if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
+      h->opt_window = (int)value;
+      return SIM_OK;
+    case SIM_OPT_ACC_REPLICAS:
+      if ((value & (value - 1)) || value > 32) return fail(h, SIM_ERR_INVALID_ARG, "replicas must be a power of two <= 32");
+      h->opt_replicas = (int)value;
+      return SIM_OK;
+    case SIM_OPT_INDEX_PATH:
+      if (value > 1) return fail(h, SIM_ERR_INVALID_ARG, "unknown index path");
+      h->opt_index_path = (int)value;
+      return SIM_OK;
+    default:
+      return fail(h, SIM_ERR_INVALID_ARG, "unknown option");
+  }
+}
+
+int sim_get_stats(const sim_handle* h, sim_stats* out) {
+  if (!h || !out) return SIM_ERR_INVALID_ARG;
+  out->kernel_launches = h->launches;
+  out->updates_accumulated = (uint64_t)h->n_updates;
+  out->scatterers_seen = h->scatterers_seen;
+  out->pulses_emitted = h->pulses_emitted;
+  return SIM_OK;
+}
+
+int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (!h_out) return fail(h, SIM_ERR_INVALID_ARG, "h_out is NULL");
+  cudaError_t e = cudaMemcpyAsync(h_out, counters(h), 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess && reset) e = cudaMemsetAsync(counters(h), 0, 4 * sizeof(uint32_t), h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "read counters");
+  return SIM_OK;
+}
+
+const char* sim_last_error(const sim_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

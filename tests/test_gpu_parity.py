@@ -1,0 +1,316 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the fp64 oracle on the same seeded
+inputs.  Spectra and IQ blocks: relative L2 <= 1e-4 (north_star); gate and bin indices: bit-exact."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2408_11472_b200 import workloads as W
+from tests import gpu_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sim_mod():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2408_11472_b200 import sim
+    sim.load_library()
+    return sim
+
+
+def _indices_exact(orc, sim_mod, wl, scat_cuda, scat_np, sim, u=0, index_path=None):
+    if index_path is not None:
+        sim.set_option(sim_mod.OPT_INDEX_PATH, index_path)
+    g0, k = sim.debug_indices(scat_cuda, sim_mod.sat_for(wl, u))
+    g0r, kr = orc.indices(U.oracle_cfg(orc, wl), U.oracle_sat(orc, wl, u), *[scat_np[f] for f in W.FIELDS[:6]])
+    assert np.array_equal(g0.cpu().numpy(), g0r), "gate indices differ from the canonical fp64 sequence"
+    assert np.array_equal(k.cpu().numpy(), kr), "Doppler-bin indices differ from the canonical fp64 sequence"
+    return int((g0r != orc.GATE_NONE).sum())
+
+
+# ---- configs[0]: Tiny, full size, every accumulation variant ----------------------------------------
+@pytest.mark.parametrize("variant", [0, 1])
+def test_tiny_full(oracle, sim_mod, variant):
+    wl = W.get("tiny")
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    T, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda, options={sim_mod.OPT_ACC_VARIANT: variant})
+    eT, eY = U.check_stream(oracle, wl, T, iq, T_ref)
+    assert eT < 2e-5 and eY < 2e-5          # the arithmetic bound derived in DESIGN.md, well inside 1e-4
+    n_in = _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
+    assert n_in == wl.n_scatterers           # the whole tiny patch is illuminated
+
+
+# ---- reduced-size versions of configs[1], [2], [4]: several tiles, ragged tail, out-of-window -------
+CASES = {
+    # nadir patch recipe, 1M scatterers (not a multiple of the 2048-scatterer chunk)
+    "nadir_1m": W.get("nadir_patch_16m").scaled(n_along=1000, n_cross=1021, n_updates=3),
+    # SAR footprint recipe (PM sea), 512 x 512 at 32 m spacing: spans the whole 16 km footprint, ~57 % in window
+    "sar_pm_coarse": W.get("sar_footprint_268m").scaled(n_along=512, n_cross=512, spacing_m=32.0, n_updates=2),
+    # SAR footprint recipe at 1 m spacing, 1024 x 1024
+    "sar_pm_1m": W.get("sar_footprint_268m").scaled(n_along=1024, n_cross=1024, n_updates=2),
+    # track strip recipe: 6 updates, satellite advancing
+    "track_small": W.get("track_segment_67m").scaled(n_along=2048, n_cross=256, n_updates=6),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_reduced_configs(oracle, sim_mod, name):
+    wl = CASES[name]
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    assert np.abs(T_ref).max() > 0
+    for variant in (0, 1):
+        T, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda, options={sim_mod.OPT_ACC_VARIANT: variant})
+        U.check_stream(oracle, wl, T, iq, T_ref)
+    for u in (0, wl.n_updates - 1):
+        _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=u)
+
+
+# ---- configs[3]: update-interval sweep, P = N in {16..512} ------------------------------------------
+@pytest.mark.parametrize("P", [16, 32, 64, 128, 256, 512])
+def test_sweep(oracle, sim_mod, P):
+    wl = W.get(f"sweep_p{P}").scaled(n_along=512, n_cross=512, n_updates=3)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    T, iq, _ = U.gpu_run(sim_mod, wl, scat_cuda)
+    U.check_stream(oracle, wl, T, iq, T_ref)
+
+
+# ---- full sizes, in the launch configuration bench.py times ----------------------------------------
+def test_full_nadir_patch_16m(oracle, sim_mod):
+    wl = W.get("nadir_patch_16m")
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    sim = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=2))
+    for u in (0, wl.n_updates - 1):
+        T_ref = U.oracle_spectra(oracle, wl, scat_np, [u])[0]
+        sim2 = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=2))
+        sim2.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
+        e = U.rel_l2(sim2.get_spectrum(0).cpu().numpy(), T_ref)
+        assert e <= U.TOL, f"update {u}: {e}"
+        _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=u)
+
+
+def test_full_sar_footprint_268m(oracle, sim_mod):
+    """configs[2] at full size (268M scatterers, 7.5 GB): one update against the full oracle
+    (all host cores), all 268M index pairs bit-exact."""
+    wl = W.get("sar_footprint_268m")
+    scat_cuda = W.scatterers(wl, device="cuda")
+    scat_np = U.to_numpy(scat_cuda)
+    u = 1
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [u])[0]
+    sim = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=2))
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
+    e = U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref)
+    assert e <= U.TOL, f"rel L2 {e}"
+    n_in = _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=u)
+    frac = n_in / wl.n_scatterers
+    assert 0.5 < frac < 0.65, frac          # pi * 6985^2 / 16384^2 = 0.57 (DESIGN.md input recipe)
+
+
+# ---- stream semantics --------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("N,P", [(64, 64), (64, 48), (32, 100), (128, 64)])
+def test_weights_and_n_not_p(oracle, sim_mod, mode, N, P):
+    wl = W.get("tiny").scaled(n_along=128, n_cross=128, n_doppler=N, pulses_per_update=P, n_updates=4)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates), weight_mode=mode)
+    T, iq, _ = U.gpu_run(sim_mod, wl, scat_cuda, weight_mode=mode)
+    U.check_stream(oracle, wl, T, iq, T_ref, weight_mode=mode)
+
+
+def test_piecewise_synthesis_equals_one_shot(oracle, sim_mod):
+    wl = W.get("tiny").scaled(n_along=64, n_cross=64, n_updates=5)
+    scat_cuda = U.to_cuda(W.scatterers(wl))
+    _, iq_all, _ = U.gpu_run(sim_mod, wl, scat_cuda)
+    for step in (1, 7, 64, 100):
+        _, iq, _ = U.gpu_run(sim_mod, wl, scat_cuda, pulses_per_call=step)
+        assert np.array_equal(iq, iq_all), f"step {step}"
+
+
+def test_streaming_ring_not_ready_overflow_and_tail(oracle, sim_mod):
+    wl = W.get("tiny").scaled(n_along=64, n_cross=64, n_updates=6)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    P, G = wl.pulses_per_update, wl.n_gates
+    sim = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=2))
+    with pytest.raises(sim_mod.SimError) as ei:
+        sim.synthesize_pulses(1)
+    assert ei.value.code == sim_mod.ERR_NOT_READY
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+    with pytest.raises(sim_mod.SimError) as ei:
+        sim.synthesize_pulses(P)                      # successor missing, no FINAL
+    assert ei.value.code == sim_mod.ERR_NOT_READY and sim.stats()["pulses_emitted"] == 0
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 1))
+    with pytest.raises(sim_mod.SimError) as ei:
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 2))   # ring of 2 is full
+    assert ei.value.code == sim_mod.ERR_OVERFLOW and sim.stats()["updates_accumulated"] == 2
+    blocks = [sim.synthesize_pulses(P)]
+    for u in range(2, wl.n_updates):                  # steady state: one update in, one segment out
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
+        blocks.append(sim.synthesize_pulses(P))
+    with pytest.raises(sim_mod.SimError):
+        sim.synthesize_pulses(P)
+    blocks.append(sim.synthesize_pulses(P, flags=sim_mod.SYN_FINAL))   # tail rule
+    iq = torch.cat(blocks).cpu().numpy()
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    Y = oracle.synthesize(U.oracle_cfg(oracle, wl), T_ref, 0, wl.n_pulses, final=True)
+    for s in range(wl.n_updates):
+        assert U.rel_l2(iq[s * P:(s + 1) * P], Y[s * P:(s + 1) * P]) <= U.TOL
+    assert sim.stats()["pulses_emitted"] == wl.n_pulses
+
+
+def test_append_equals_single_call_and_linearity(oracle, sim_mod):
+    wl = W.get("tiny").scaled(n_along=200, n_cross=203, n_updates=1)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    cut = 12345 // 4 * 4                                # 16-byte aligned split of the device arrays
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    sat = sim_mod.sat_for(wl, 0)
+    with pytest.raises(sim_mod.SimError):
+        sim.accumulate_update({k: v[:cut] for k, v in scat_cuda.items()}, sat, flags=sim_mod.ACC_APPEND)
+    sim.accumulate_update({k: v[:cut] for k, v in scat_cuda.items()}, sat)
+    sim.accumulate_update({k: v[cut:] for k, v in scat_cuda.items()}, sat, flags=sim_mod.ACC_APPEND)
+    assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
+    assert sim.stats()["updates_accumulated"] == 1
+
+
+# ---- edge cases ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [0, 1, 3, 4, 5, 2047, 2048, 2049, 3 * 2048 + 5])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_ragged_sizes(oracle, sim_mod, n, variant):
+    wl = W.get("tiny").scaled(n_updates=1)
+    scat = {k: v[:n].contiguous() for k, v in W.scatterers(wl).items()}
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+    T = sim.get_spectrum(0).cpu().numpy()
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0] if n else np.zeros_like(T)
+    assert U.rel_l2(T, T_ref) <= U.TOL
+    if n:
+        _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_degenerate_inputs(oracle, sim_mod, variant):
+    """Out-of-window, dead (s0dA <= 0, NaN), non-finite positions/velocities: dropped on both sides."""
+    wl = W.get("tiny").scaled(n_updates=1)
+    scat = {k: v[:8192].clone() for k, v in W.scatterers(wl).items()}
+    scat["z"][0:500] = 100.0                      # far out of the window (too near)
+    scat["z"][500:1000] = -100.0                  # too far
+    scat["s0dA"][1000:1500] = 0.0
+    scat["s0dA"][1500:1600] = -3.0
+    scat["s0dA"][1600:1700] = float("nan")
+    scat["x"][1700:1800] = float("nan")
+    scat["vz"][1800:1900] = float("inf")
+    scat["z"][1900:2000] = 64 // 2 * 0.468 + 0.2  # gf in [-1,0): only the upper half lands (gate 0)
+    scat["z"][2000:2100] = -(31 * 0.468 + 0.2)    # gf in [G-1,G): only the lower half lands
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+    T = sim.get_spectrum(0).cpu().numpy()
+    assert np.all(np.isfinite(T.view(np.float32)))
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    assert U.rel_l2(T, T_ref) <= U.TOL
+    assert np.abs(T_ref[0]).max() > 0 and np.abs(T_ref[63]).max() > 0
+    _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
+    # nothing illuminated at all: the spectrum must be exactly zero (reading A17)
+    dead = {k: v.clone() for k, v in scat_cuda.items()}
+    dead["z"][:] = 500.0
+    sim.accumulate_update(dead, sim_mod.sat_for(wl, 0))
+    assert torch.count_nonzero(torch.view_as_real(sim.get_spectrum(1))) == 0
+
+
+def test_shuffled_order_and_tiny_window(oracle, sim_mod):
+    """The shared-memory window is an optimisation, not an assumption: randomly ordered scatterers and a
+    1-bin window (everything else through the global-atomic path) give the same spectrum."""
+    wl = W.get("nadir_patch_16m").scaled(n_along=300, n_cross=300, n_updates=1)
+    scat = W.scatterers(wl)
+    perm = torch.randperm(wl.n_scatterers, generator=torch.Generator().manual_seed(1))
+    scat = {k: v[perm].contiguous() for k, v in scat.items()}
+    scat["vz"] *= 40.0                                  # spread over many Doppler bins
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    assert (np.abs(T_ref).max(axis=0) > 0).sum() > 60
+    for opts in ({}, {sim_mod.OPT_ACC_WINDOW_BINS: 1, sim_mod.OPT_ACC_REPLICAS: 1},
+                 {sim_mod.OPT_ACC_SUPERCHUNK: 2048, sim_mod.OPT_ACC_BLOCKS: 7}):
+        sim = sim_mod.Sim(sim_mod.config_for(wl))
+        for k, v in opts.items():
+            sim.set_option(k, v)
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+        assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
+        if opts.get(sim_mod.OPT_ACC_WINDOW_BINS) == 1:
+            assert sim.read_counters()["window_misses"] > 0
+
+
+def test_maximum_sizes(oracle, sim_mod):
+    wl = W.get("tiny").scaled(n_along=256, n_cross=256, n_gates=1024, n_doppler=1024, pulses_per_update=1024,
+                              n_updates=2, gate_spacing_m=0.05)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    T, iq, _ = U.gpu_run(sim_mod, wl, scat_cuda)
+    U.check_stream(oracle, wl, T, iq, T_ref)
+
+
+def test_off_nadir_boresight_and_isotropic(oracle, sim_mod):
+    wl = W.get("nadir_patch_16m").scaled(n_along=256, n_cross=256, n_updates=1)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    for alpha, bore in ((wl.antenna_alpha, (0.004, -0.002, -1.0)), (0.0, (0.0, 0.0, -2.0))):
+        wl2 = wl.scaled(antenna_alpha=alpha)
+        s = W.sat_state(wl2, 0)
+        T_ref, _ = oracle.spectrum(U.oracle_cfg(oracle, wl2), oracle.make_sat(s["pos"], s["vel"], bore, s["range_gate0_m"]),
+                                   *[scat_np[f] for f in W.FIELDS])
+        sim = sim_mod.Sim(sim_mod.config_for(wl2))
+        sim.accumulate_update(scat_cuda, sim_mod.make_sat(s["pos"], s["vel"], bore, s["range_gate0_m"]))
+        assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
+
+
+def test_host_buffer_entry_points(oracle, sim_mod):
+    wl = W.get("tiny").scaled(n_along=300, n_cross=301, n_updates=3)
+    scat = W.scatterers(wl)
+    scat_np = U.to_numpy(scat)
+    pinned = {k: v.pin_memory() for k, v in scat.items()}
+    cfg = sim_mod.config_for(wl, max_pending_updates=4, host_stage_scatterers=20000, host_stage_pulses=wl.n_pulses)
+    sim = sim_mod.Sim(cfg)
+    for u in range(wl.n_updates):
+        sim.accumulate_update_host(pinned, sim_mod.sat_for(wl, u))
+    iq = torch.empty((wl.n_pulses, wl.n_gates), dtype=torch.complex64).pin_memory()
+    sim.synthesize_pulses_host(wl.n_pulses, iq, flags=sim_mod.SYN_FINAL)
+    sim.synchronize()
+    T = torch.stack([sim.get_spectrum(u) for u in range(wl.n_updates)]).cpu().numpy()
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    U.check_stream(oracle, wl, T, iq.numpy(), T_ref)
+
+
+def test_argument_errors(sim_mod):
+    wl = W.get("tiny")
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    scat = U.to_cuda({k: v[:4096] for k, v in W.scatterers(wl).items()})
+    bad = dict(scat)
+    bad["y"] = scat["y"][1:]                         # misaligned and wrong length
+    with pytest.raises(ValueError):
+        sim.accumulate_update(bad, sim_mod.sat_for(wl, 0))
+    bad = {k: v[1:4001] for k, v in scat.items()}    # 4-byte offset: not 16-byte aligned
+    with pytest.raises(sim_mod.SimError) as ei:
+        sim.accumulate_update(bad, sim_mod.sat_for(wl, 0))
+    assert ei.value.code == sim_mod.ERR_INVALID_ARG
+    with pytest.raises(sim_mod.SimError):
+        sim.accumulate_update(scat, sim_mod.make_sat((0, 0, 1), (0, 0, 0), (0, 0, 0), 0.0))   # zero boresight
+    with pytest.raises(sim_mod.SimError):
+        sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, 3)
+    assert sim.stats()["updates_accumulated"] == 0   # errors leave the handle unchanged
+    sim.accumulate_update(scat, sim_mod.sat_for(wl, 0))
+    assert sim.stats()["updates_accumulated"] == 1 and sim.stats()["kernel_launches"] >= 2
