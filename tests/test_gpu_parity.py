@@ -133,7 +133,8 @@ def test_piecewise_synthesis_equals_one_shot(oracle, sim_mod):
     _, iq_all, _ = U.gpu_run(sim_mod, wl, scat_cuda)
     for step in (1, 7, 64, 100):
         _, iq, _ = U.gpu_run(sim_mod, wl, scat_cuda, pulses_per_call=step)
-        assert np.array_equal(iq, iq_all), f"step {step}"
+        # every run re-accumulates with fp32 atomics (order not deterministic): equal up to that rounding
+        assert U.rel_l2(iq, iq_all) <= 1e-5, f"step {step}"
 
 
 def test_streaming_ring_not_ready_overflow_and_tail(oracle, sim_mod):
