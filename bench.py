@@ -362,7 +362,8 @@ def main():
             "iq_samples_per_s": iq_rate,
             "split_ms": {"accumulate_per_update": acc_ms_mean, "synthesize_per_step": syn_ms},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches,
-            "clocks": clk.summary(), "window_misses_per_step": counters["window_misses"] / max(1, args.steps),
+            "clocks": clk.summary(), "escapes_per_step": counters["escapes"] / max(1, args.steps),
+            "index_fallbacks_per_step": counters["index_fallbacks"] / max(1, args.steps),
         }
         print(json.dumps(out), flush=True)
     if world > 1:

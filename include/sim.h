@@ -158,15 +158,16 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto */
 #define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit; 0 = auto */
 #define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto */
-#define SIM_OPT_ACC_REPLICAS 5  /* shared-memory replicas of the tile; 0 = auto */
-#define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band */
+#define SIM_OPT_GUARD_LSB 5     /* guard band of the fast index path in units of 2^-20 gate / bin (default 16) */
+#define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 
 int sim_get_stats(const sim_handle* h, sim_stats* out);
 
 /* Synchronises the stream, copies the library's device counters to h_out (HOST, 4 x uint32:
- * [0] scheduling tickets of the last accumulation launch, [1] contributions that missed the
- * shared-memory window and went to global atomics, [2] tile flushes, [3] reserved) and, when
+ * [0] scheduling tickets of the last accumulation launch, [1] scatterers whose contributions left the
+ * shared-memory tile for global atomics (outside the Doppler window / above the fixed-point range),
+ * [2] tile flushes, [3] scatterers whose indices the canonical sequence decided (guard band)) and, when
  * reset != 0, zeroes them. */
 int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset);
 

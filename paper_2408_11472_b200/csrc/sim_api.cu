@@ -77,8 +77,9 @@ struct sim_handle {
   int64_t n_updates;             // spectra started so far
   int64_t pulses_emitted;
   // tuning
-  int opt_variant, opt_blocks, opt_window, opt_replicas, opt_index_path;
+  int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard;
   int64_t opt_superchunk;
+  int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
   // stats
   uint64_t launches, scatterers_seen;
   std::string err;
@@ -125,17 +126,63 @@ int check_sat(sim_handle* h, const sim_sat_state* sat) {
   return SIM_OK;
 }
 
-// Tile geometry: W Doppler bins x G gates x R replicas of float2 in shared memory.
-void choose_tile(const sim_handle* h, int* W, int* R) {
+// Shared-memory tile: W Doppler bins x G gates of (int2 + float2).  Small enough for several blocks per SM.
+int choose_window(const sim_handle* h) {
   const int G = h->cfg.n_gates, N = h->cfg.n_doppler;
-  const size_t budget = h->smem_optin > 64 * 1024 ? h->smem_optin - 16 * 1024 : 32 * 1024;
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
-  int r = h->opt_replicas > 0 ? h->opt_replicas : 8;
-  while (r > 1 && (size_t)G * w * r * sizeof(float2) > budget) r >>= 1;
-  while (w > 1 && (size_t)G * w * r * sizeof(float2) > budget) w >>= 1;
-  *W = w;
-  *R = r;
+  const size_t budget = h->opt_window > 0 ? (h->smem_optin > 8192 ? h->smem_optin - 4096 : 4096) : 64 * 1024;
+  while (w > 1 && acc_tile_smem_bytes(G, w) > budget) w >>= 1;
+  return w;
+}
+
+// Constants of the sqrt/divide-free index path and the decision whether it is valid for this geometry
+// (error bounds that the guard band must cover).
+void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParams& p) {
+  const double rg0 = sat->range_gate0_m, dR = h->cfg.gate_spacing_m, lam = h->cfg.wavelength_m;
+  const int G = h->cfg.n_gates;
+  p.guard = h->opt_guard;
+  p.fast_ok = 0;
+  {  // frac(rg0 * 2 / lambda) to ~1e-17 cycles: product split into rounded part + exact residual
+    const double c = 2.0 / lam, q = rg0 * c, qe = std::fma(rg0, c, -q);
+    p.fr0 = (q - std::floor(q)) + qe;
+  }
+  if (!(rg0 > 0)) return;
+  const double margin = 0.01 * dR + 1e-9 * rg0;
+  const double d_lo = -dR - margin, d_hi = G * dR + margin;
+  const double dmax = std::fmax(-d_lo, d_hi), emax = dmax / rg0, rmax = rg0 + d_hi;
+  if (!(rg0 + d_lo > 0) || !(emax < 1.0 / 1024.0)) return;
+  p.rg0sq_hi = rg0 * rg0;
+  p.rg0sq_lo = std::fma(rg0, rg0, -p.rg0sq_hi);
+  p.u_lo = d_lo * (2.0 * rg0 + d_lo);
+  p.u_hi = d_hi * (2.0 * rg0 + d_hi);
+  p.inv_2rg0 = 0.5 / rg0;
+  p.b1 = -0.5 / rg0;
+  p.b2 = 0.5 / (rg0 * rg0);
+  p.b3 = -0.625 / (rg0 * rg0 * rg0);
+  p.inv_rg0 = 1.0 / rg0;
+  const double c = 2.0 / lam;
+  // gate: |delta_fast - delta_canonical| <= sqrt rounding + series truncation + Horner rounding
+  const double err_m = 3e-16 * rmax + 0.06 * std::pow(2.0 * emax, 4) * dmax + 1e-15 * dmax;
+  const double guard_m = p.guard * dR / (double)(1 << kFracBits);
+  // Doppler (|kf| < 1024 on the fast path): 1/R series truncation e^4 + roundings
+  const double err_k = 1024.0 * (std::pow(emax, 4) + 2e-15);
+  const double guard_k = p.guard / (double)(1 << kFracBits);
+  const bool phase_ok = (G + 2) * dR * c < 134217728.0;   // 2^27: the magic-number fraction needs |q| < 2^28
+  if (guard_m >= 4.0 * err_m && guard_k >= 4.0 * err_k && phase_ok && G + 2 < 2048) p.fast_ok = 1;
+}
+
+int acc_blocks(const sim_handle* h) {
+  return h->opt_blocks > 0 ? h->opt_blocks : h->sm_count * (h->tile_blocks_per_sm > 0 ? h->tile_blocks_per_sm : 1);
+}
+
+// (Re)chooses the window width and the resident blocks per SM; cheap, called when an option changes.
+cudaError_t plan_tile(sim_handle* h) {
+  h->tile_W = choose_window(h);
+  int b = 1;
+  cudaError_t e = acc_tile_blocks_per_sm(h->cfg.n_gates, h->tile_W, &b);
+  h->tile_blocks_per_sm = b > 0 ? b : 1;
+  return e;
 }
 
 AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sat, float2* T) {
@@ -149,18 +196,26 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.inv_dR = 1.0 / h->cfg.gate_spacing_m;
   p.two_over_lambda = 2.0 / h->cfg.wavelength_m;
   p.cD = (-2.0 * (double)h->cfg.n_doppler) / (h->cfg.wavelength_m * h->cfg.prf_hz);
+  fast_path_constants(h, sat, p);
   const double bn = std::sqrt(sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
                               sat->boresight[2] * sat->boresight[2]);
   p.bx = (float)(sat->boresight[0] / bn);
   p.by = (float)(sat->boresight[1] / bn);
   p.bz = (float)(sat->boresight[2] / bn);
-  p.alpha = (float)h->cfg.antenna_alpha;
+  p.sxh = (float)sat->pos[0]; p.sxl = (float)(sat->pos[0] - (double)p.sxh);
+  p.syh = (float)sat->pos[1]; p.syl = (float)(sat->pos[1] - (double)p.syh);
+  p.szh = (float)sat->pos[2]; p.szl = (float)(sat->pos[2] - (double)p.szh);
+  p.neg_alpha_log2e = (float)(-h->cfg.antenna_alpha * 1.4426950408889634);
+  p.dR_fx = (float)(h->cfg.gate_spacing_m / (double)(1 << kFracBits));
+  p.dR_f = (float)h->cfg.gate_spacing_m;
+  p.inv_rg0_f = (float)(1.0 / sat->range_gate0_m);
+  p.inv_rg0sq_f = (float)(1.0 / (sat->range_gate0_m * sat->range_gate0_m));
   p.G = h->cfg.n_gates;
   p.N = h->cfg.n_doppler;
   p.T = T;
   p.counters = counters(h);
-  choose_tile(h, &p.W, &p.R);
-  const int blocks = h->opt_blocks > 0 ? h->opt_blocks : h->sm_count;
+  p.W = h->tile_W;
+  const int blocks = acc_blocks(h);
   unsigned long long sc = (unsigned long long)h->opt_superchunk;
   if (sc == 0) {
     // aim at >= 8 scheduling units per block, between one chunk and 64K scatterers
@@ -175,7 +230,7 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
 
 int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, float2* T) {
   AccParams p = make_acc_params(h, d_scat, sat, T);
-  const int blocks = h->opt_blocks > 0 ? h->opt_blocks : h->sm_count;
+  const int blocks = acc_blocks(h);
   int l = 0;
   cudaError_t e = launch_accumulate(p, h->opt_variant, blocks, h->stream, &l);
   h->launches += l;
@@ -282,8 +337,10 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->opt_variant = 1;
   h->opt_blocks = 0;
   h->opt_window = 0;
-  h->opt_replicas = 0;
-  h->opt_index_path = 0;
+  h->opt_index_path = 1;
+  h->opt_guard = 16;
+  h->tile_W = 0;
+  h->tile_blocks_per_sm = 0;
   h->opt_superchunk = 0;
   h->launches = 0;
   h->scatterers_seen = 0;
@@ -302,6 +359,8 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
       cudaEventCreateWithFlags(&h->ev_consumed[b], cudaEventDisableTiming);
     }
   }
+  e = plan_tile(h);
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters)"); }
   int l = 0;
@@ -467,10 +526,11 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       if (value & (value - 1)) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two");
       if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
       h->opt_window = (int)value;
+      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;
-    case SIM_OPT_ACC_REPLICAS:
-      if ((value & (value - 1)) || value > 32) return fail(h, SIM_ERR_INVALID_ARG, "replicas must be a power of two <= 32");
-      h->opt_replicas = (int)value;
+    case SIM_OPT_GUARD_LSB:
+      if (value < 1 || value > (1 << (kFracBits - 2))) return fail(h, SIM_ERR_INVALID_ARG, "guard must be in 1..2^18");
+      h->opt_guard = (int)value;
       return SIM_OK;
     case SIM_OPT_INDEX_PATH:
       if (value > 1) return fail(h, SIM_ERR_INVALID_ARG, "unknown index path");

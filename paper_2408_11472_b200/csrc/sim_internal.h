@@ -7,35 +7,53 @@
 
 namespace simk {
 
-constexpr int kAccThreads = 512;              // threads per block of the accumulation kernels
+constexpr int kAccThreads = 256;              // threads per block of the tile accumulation kernel
+constexpr int kAccWarps = kAccThreads / 32;
 constexpr int kAccPerThread = 4;              // scatterers per thread per chunk (one 128-bit load per array)
-constexpr int kAccChunk = kAccThreads * kAccPerThread;
+constexpr int kAccChunk = kAccThreads * kAccPerThread;  // = one fixed-point epoch (1024 scatterers)
 constexpr int kNumCounters = 64;
+constexpr int kFracBits = 20;                 // fixed-point fraction bits of the gate / Doppler coordinates
 
 enum Counter : int {
-  kCtrTicket = 0,   // super-chunk ticket of the running accumulation launch
-  kCtrMiss = 1,     // contributions that fell outside the shared-memory window (global atomics)
-  kCtrFlush = 2,    // tile flushes
+  kCtrTicket = 0,   // scheduling ticket of the running accumulation launch
+  kCtrEscape = 1,   // contributions sent to global atomics (outside the window or above the fixed-point range)
+  kCtrFlush = 2,    // fp32 tile flushes (window moves + final)
+  kCtrFallback = 3, // scatterers whose indices were decided by the canonical sequence (guard band)
 };
 
 // Everything the accumulation kernels need, passed by value.
 struct AccParams {
   const float *x, *y, *z, *vx, *vy, *vz, *s0dA;
   unsigned long long n;
+  // ---- canonical fp64 sequence ----
   double sx, sy, sz;      // satellite position
   double svx, svy, svz;   // satellite velocity
   double rg0;             // range of the centre of gate 0
   double inv_dR;          // 1.0 / gate_spacing
   double two_over_lambda; // 2.0 / wavelength
   double cD;              // (-2.0 * N) / (wavelength * PRF)
-  float bx, by, bz;       // unit boresight
-  float alpha;            // antenna_alpha
+  // ---- fast index path: delta = R - rg0 from u = R^2 - rg0^2 by series, no sqrt / div ----
+  double rg0sq_hi, rg0sq_lo;  // rg0^2 as an exact double-double
+  double u_lo, u_hi;          // u outside [u_lo, u_hi] is certainly outside the gate window
+  double inv_2rg0;            // 1 / (2 rg0)
+  double b1, b2, b3;          // delta = t (1 + t (b1 + t (b2 + t b3))),  t = u / (2 rg0)
+  double inv_rg0;             // 1 / rg0
+  double fr0;                 // frac(rg0 * 2 / lambda), exact to ~1e-17
+  int guard;                  // guard band in units of 2^-kFracBits around integer gate / bin boundaries
+  int fast_ok;                // host-side validity of the fast path for this geometry
+  // ---- fp32 amplitude path ----
+  float sxh, sxl, syh, syl, szh, szl;  // satellite position as float hi + lo
+  float bx, by, bz;                    // unit boresight
+  float neg_alpha_log2e;               // -antenna_alpha * log2(e)
+  float dR_fx;                         // gate_spacing * 2^-kFracBits
+  float dR_f;                          // gate_spacing
+  float inv_rg0_f;                     // 1 / rg0
+  float inv_rg0sq_f;                   // 1 / rg0^2
   int G, N;
   float2* T;              // spectrum of the current update, [G][N]
   unsigned int* counters; // kNumCounters device words
   unsigned long long superchunk; // scatterers per scheduling unit (multiple of kAccChunk)
-  int W;                  // window bins in shared memory (power of two, <= N)
-  int R;                  // replicas (power of two)
+  int W;                  // Doppler bins of the shared-memory window (power of two, <= N)
   int index_path;         // 0 canonical everywhere, 1 fast path + guard band
 };
 
@@ -58,7 +76,8 @@ cudaError_t launch_accumulate(const AccParams& p, int variant, int blocks, cudaS
                               int* launches);
 cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
                            int* launches);
-cudaError_t acc_tile_smem_bytes(int G, int W, int R, size_t* bytes);
+size_t acc_tile_smem_bytes(int G, int W);
+cudaError_t acc_tile_blocks_per_sm(int G, int W, int* blocks);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
 int synth_gate_tile(int N);

@@ -19,7 +19,7 @@ W_SQRT, W_LINEAR = 0, 1
 ACC_APPEND = 1
 SYN_FINAL = 1
 GATE_NONE = -(2**31)
-OPT_ACC_VARIANT, OPT_ACC_BLOCKS, OPT_ACC_SUPERCHUNK, OPT_ACC_WINDOW_BINS, OPT_ACC_REPLICAS, OPT_INDEX_PATH = 1, 2, 3, 4, 5, 6
+OPT_ACC_VARIANT, OPT_ACC_BLOCKS, OPT_ACC_SUPERCHUNK, OPT_ACC_WINDOW_BINS, OPT_GUARD_LSB, OPT_INDEX_PATH = 1, 2, 3, 4, 5, 6
 
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",
@@ -229,7 +229,7 @@ class Sim:
     def read_counters(self, reset: bool = False) -> dict:
         a = (C.c_uint32 * 4)()
         self._check(self.lib.sim_read_counters(self._h, a, int(reset)), self._h)
-        return {"tickets": a[0], "window_misses": a[1], "flushes": a[2]}
+        return {"tickets": a[0], "escapes": a[1], "flushes": a[2], "index_fallbacks": a[3]}
 
 
 def config_for(wl, **kw) -> SimConfig:

@@ -244,7 +244,7 @@ def test_shuffled_order_and_tiny_window(oracle, sim_mod):
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
     assert (np.abs(T_ref).max(axis=0) > 0).sum() > 60
-    for opts in ({}, {sim_mod.OPT_ACC_WINDOW_BINS: 1, sim_mod.OPT_ACC_REPLICAS: 1},
+    for opts in ({}, {sim_mod.OPT_ACC_WINDOW_BINS: 1}, {sim_mod.OPT_ACC_WINDOW_BINS: 4},
                  {sim_mod.OPT_ACC_SUPERCHUNK: 2048, sim_mod.OPT_ACC_BLOCKS: 7}):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
         for k, v in opts.items():
@@ -252,7 +252,82 @@ def test_shuffled_order_and_tiny_window(oracle, sim_mod):
         sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
         assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
         if opts.get(sim_mod.OPT_ACC_WINDOW_BINS) == 1:
-            assert sim.read_counters()["window_misses"] > 0
+            assert sim.read_counters()["escapes"] > 0
+
+
+def test_guard_band_and_exact_boundaries(oracle, sim_mod):
+    """Fast index path: (i) scatterers sitting EXACTLY on gate boundaries and on Doppler-bin ties are
+    decided by the canonical sequence (bit-exact indices); (ii) any guard width gives the same indices;
+    (iii) the canonical-only path (index_path 0) gives the same spectrum."""
+    wl = W.get("tiny").scaled(n_updates=1, gate_spacing_m=0.5)        # dyadic gate spacing
+    n = 4096
+    scat = {k: v[:n].clone() for k, v in W.scatterers(wl).items()}
+    rg0 = wl.range_gate0_m                                            # 814500 - 16: an integer
+    m = torch.arange(n) % 48
+    scat["x"][:] = 0.0
+    scat["y"][:] = 0.0
+    scat["z"][:] = (814500.0 - rg0) - 0.5 * m.float()                 # R - rg0 = m * dR exactly
+    scat["vx"][:] = 7000.0                                            # no relative horizontal motion
+    scat["vy"][:] = 0.0
+    # vertical speed on exact half-bins: kf = j + 0.5 (ties round up), dyadic so that fp32 holds it
+    lam_prf = wl.wavelength_m * wl.prf_hz / (2 * wl.n_doppler)
+    scat["vz"][:] = ((torch.arange(n) % 7).float() - 3.0) * 0.5 * float(np.float32(lam_prf))
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    sat_args = ((0.0, 0.0, 814500.0), (7000.0, 0.0, 0.0), (0.0, 0.0, -1.0), rg0)   # satellite exactly overhead
+    g0r, kr = oracle.indices(U.oracle_cfg(oracle, wl), oracle.make_sat(*sat_args), *[scat_np[f] for f in W.FIELDS[:6]])
+    assert np.array_equal(g0r, m.numpy())                             # gf is exactly the integer m
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    for path, guard in ((1, 16), (1, 1), (1, 4096), (1, 1 << 18), (0, 16)):
+        sim.set_option(sim_mod.OPT_INDEX_PATH, path)
+        sim.set_option(sim_mod.OPT_GUARD_LSB, guard)
+        sim.read_counters(reset=True)
+        g0, k = sim.debug_indices(scat_cuda, sim_mod.make_sat(*sat_args))
+        assert np.array_equal(g0.cpu().numpy(), g0r) and np.array_equal(k.cpu().numpy(), kr), (path, guard)
+        fb = sim.read_counters()["index_fallbacks"]
+        assert (fb == n) if path == 1 else (fb == 0)                  # every one of them is a boundary case
+    # (ii)/(iii) on an ordinary scene
+    wl = W.get("nadir_patch_16m").scaled(n_along=512, n_cross=512, n_updates=1)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    for path, guard in ((1, 16), (1, 1 << 18), (1, 30000), (0, 16)):
+        sim = sim_mod.Sim(sim_mod.config_for(wl))
+        sim.set_option(sim_mod.OPT_INDEX_PATH, path)
+        sim.set_option(sim_mod.OPT_GUARD_LSB, guard)
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+        assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
+        _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
+        fb = sim.read_counters()["index_fallbacks"]
+        if path == 1 and guard == 16:
+            assert fb < 1e-3 * wl.n_scatterers                        # the guard band is thin
+        if path == 1 and guard == 1 << 18:
+            assert fb > 0.9 * wl.n_scatterers
+
+
+def test_heavy_tailed_amplitudes(oracle, sim_mod):
+    """Block-floating-point accumulation: bright targets 10^6 x the sea (they leave the int32 range and take
+    the exact global-atomic path), dead zones, and amplitude steps between chunks keep the 1e-4 bound."""
+    wl = W.get("nadir_patch_16m").scaled(n_along=256, n_cross=1024, n_updates=1)
+    scat = W.scatterers(wl)
+    g = torch.Generator().manual_seed(3)
+    s0 = scat["s0dA"]
+    bright = torch.randperm(s0.numel(), generator=g)[:300]
+    s0[bright] *= 1e12                                               # amplitude x 1e6
+    s0[50_000:80_000] *= 1e-8                                        # a dark band (amplitude x 1e-4)
+    s0[120_000:121_024] = 0.0                                        # a dead chunk
+    s0[200_000:] *= torch.exp(4.0 * torch.randn(s0.numel() - 200_000, generator=g))   # lognormal, sigma 2 in amplitude
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+    assert U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref) <= U.TOL
+    assert sim.read_counters()["escapes"] >= 300
+    # the dark band alone (a scene that is dim everywhere) is resolved just as well
+    dim = {k: v[50_000:80_000 - 16].contiguous() for k, v in scat_cuda.items()}
+    dim_np = U.to_numpy(dim)
+    T_ref = U.oracle_spectra(oracle, wl, dim_np, [0])[0]
+    sim.accumulate_update(dim, sim_mod.sat_for(wl, 0))
+    assert U.rel_l2(sim.get_spectrum(1).cpu().numpy(), T_ref) <= U.TOL
 
 
 def test_maximum_sizes(oracle, sim_mod):
