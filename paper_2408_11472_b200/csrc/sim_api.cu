@@ -77,7 +77,7 @@ struct sim_handle {
   int64_t n_updates;             // spectra started so far
   int64_t pulses_emitted;
   // tuning
-  int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard;
+  int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard, opt_per_thread, opt_min_blocks;
   int64_t opt_superchunk;
   int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
   // stats
@@ -126,13 +126,16 @@ int check_sat(sim_handle* h, const sim_sat_state* sat) {
   return SIM_OK;
 }
 
-// Shared-memory tile: W Doppler bins x G gates of (int2 + float2).  Small enough for several blocks per SM.
+// Shared-memory tile: W Doppler bins x G gates of int2, next to the two input stages.  Small enough for
+// several blocks per SM.
 int choose_window(const sim_handle* h) {
   const int G = h->cfg.n_gates, N = h->cfg.n_doppler;
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
-  const size_t budget = h->opt_window > 0 ? (h->smem_optin > 8192 ? h->smem_optin - 4096 : 4096) : 64 * 1024;
-  while (w > 1 && acc_tile_smem_bytes(G, w) > budget) w >>= 1;
+  // default: at most 32 KB of tile next to the stages; an explicit window may use all of shared memory
+  const size_t stages = acc_tile_smem_bytes(0, 0, h->opt_per_thread);
+  const size_t budget = h->opt_window > 0 ? (h->smem_optin > 8192 ? h->smem_optin - 4096 : 4096) : stages + 32 * 1024;
+  while (w > 1 && acc_tile_smem_bytes(G, w, h->opt_per_thread) > budget) w >>= 1;
   return w;
 }
 
@@ -170,6 +173,12 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
   const double guard_k = p.guard / (double)(1 << kFracBits);
   const bool phase_ok = (G + 2) * dR * c < 134217728.0;   // 2^27: the magic-number fraction needs |q| < 2^28
   if (guard_m >= 4.0 * err_m && guard_k >= 4.0 * err_k && phase_ok && G + 2 < 2048) p.fast_ok = 1;
+  // fp32 pre-test: |u_f32 - u| <= 2^-21 R^2 (three squares, two sums, the split satellite position and
+  // rg0^2 each rounded to 2^-24); the margin is twice that at the far edge of the window
+  const double margin_u = std::ldexp(rmax * rmax, -20);
+  p.rg0sq_f = (float)(rg0 * rg0);
+  p.uf_lo = (float)(p.u_lo - margin_u);
+  p.uf_hi = (float)(p.u_hi + margin_u);
 }
 
 int acc_blocks(const sim_handle* h) {
@@ -180,7 +189,7 @@ int acc_blocks(const sim_handle* h) {
 cudaError_t plan_tile(sim_handle* h) {
   h->tile_W = choose_window(h);
   int b = 1;
-  cudaError_t e = acc_tile_blocks_per_sm(h->cfg.n_gates, h->tile_W, &b);
+  cudaError_t e = acc_tile_blocks_per_sm(h->cfg.n_gates, h->tile_W, h->opt_per_thread, h->opt_min_blocks, &b);
   h->tile_blocks_per_sm = b > 0 ? b : 1;
   return e;
 }
@@ -232,7 +241,7 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
   AccParams p = make_acc_params(h, d_scat, sat, T);
   const int blocks = acc_blocks(h);
   int l = 0;
-  cudaError_t e = launch_accumulate(p, h->opt_variant, blocks, h->stream, &l);
+  cudaError_t e = launch_accumulate(p, h->opt_variant, h->opt_per_thread, h->opt_min_blocks, blocks, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
@@ -339,6 +348,8 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->opt_window = 0;
   h->opt_index_path = 1;
   h->opt_guard = 16;
+  h->opt_per_thread = 4;
+  h->opt_min_blocks = 3;
   h->tile_W = 0;
   h->tile_blocks_per_sm = 0;
   h->opt_superchunk = 0;
@@ -526,6 +537,16 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       if (value & (value - 1)) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two");
       if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
       h->opt_window = (int)value;
+      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      return SIM_OK;
+    case SIM_OPT_ACC_PER_THREAD:
+      if (value != 2 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "scatterers per thread must be 2 or 4");
+      h->opt_per_thread = (int)value;
+      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      return SIM_OK;
+    case SIM_OPT_ACC_MIN_BLOCKS:
+      if (value < 2 || value > 4) return fail(h, SIM_ERR_INVALID_ARG, "register budget: 2..4 blocks per SM");
+      h->opt_min_blocks = (int)value;
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;
     case SIM_OPT_GUARD_LSB:

@@ -9,15 +9,14 @@ namespace simk {
 
 constexpr int kAccThreads = 256;              // threads per block of the tile accumulation kernel
 constexpr int kAccWarps = kAccThreads / 32;
-constexpr int kAccPerThread = 4;              // scatterers per thread per chunk (one 128-bit load per array)
-constexpr int kAccChunk = kAccThreads * kAccPerThread;  // = one fixed-point epoch (1024 scatterers)
+constexpr int kAccChunk = kAccThreads * 4;    // largest chunk (4 scatterers per thread) = one fixed-point epoch
 constexpr int kNumCounters = 64;
 constexpr int kFracBits = 20;                 // fixed-point fraction bits of the gate / Doppler coordinates
 
 enum Counter : int {
   kCtrTicket = 0,   // scheduling ticket of the running accumulation launch
   kCtrEscape = 1,   // contributions sent to global atomics (outside the window or above the fixed-point range)
-  kCtrFlush = 2,    // fp32 tile flushes (window moves + final)
+  kCtrFlush = 2,    // unused (the tile drains to global every epoch)
   kCtrFallback = 3, // scatterers whose indices were decided by the canonical sequence (guard band)
 };
 
@@ -49,6 +48,7 @@ struct AccParams {
   float dR_f;                          // gate_spacing
   float inv_rg0_f;                     // 1 / rg0
   float inv_rg0sq_f;                   // 1 / rg0^2
+  float rg0sq_f, uf_lo, uf_hi;         // fp32 pre-test: u_f32 = R^2 - rg0^2 outside [uf_lo, uf_hi] is certainly out
   int G, N;
   float2* T;              // spectrum of the current update, [G][N]
   unsigned int* counters; // kNumCounters device words
@@ -72,12 +72,12 @@ struct SynParams {
   int weight_mode;
 };
 
-cudaError_t launch_accumulate(const AccParams& p, int variant, int blocks, cudaStream_t st,
-                              int* launches);
+cudaError_t launch_accumulate(const AccParams& p, int variant, int per_thread, int min_blocks, int blocks,
+                              cudaStream_t st, int* launches);
 cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
                            int* launches);
-size_t acc_tile_smem_bytes(int G, int W);
-cudaError_t acc_tile_blocks_per_sm(int G, int W, int* blocks);
+size_t acc_tile_smem_bytes(int G, int W, int per_thread);
+cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
 int synth_gate_tile(int N);
