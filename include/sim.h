@@ -154,13 +154,16 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
                       int32_t* d_gate0, int32_t* d_bin);
 
 /* Tuning knobs (benchmarks and tests; defaults are chosen by the library). */
-#define SIM_OPT_ACC_VARIANT 1   /* 0 = reference kernel (global atomics), 1 = shared-memory tile kernel */
+#define SIM_OPT_ACC_VARIANT 1   /* 0 = reference kernel (global atomics), 1 = barrier-synchronised tile kernel,
+                                   2 = warp-specialised tile kernel (default) */
 #define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto */
 #define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit; 0 = auto */
 #define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto */
 #define SIM_OPT_GUARD_LSB 5     /* guard band of the fast index path in units of 2^-20 gate / bin (default 16) */
 #define SIM_OPT_ACC_PER_THREAD 7 /* scatterers per thread per chunk of the tile kernel: 2 or 4 */
 #define SIM_OPT_ACC_MIN_BLOCKS 8 /* register budget of the tile kernel: compiled for 2..4 resident blocks per SM */
+#define SIM_OPT_ACC_WARPS 9      /* variant 2: compute warps per block: 7, 14 (default), 22 or 30 */
+#define SIM_OPT_ACC_STAGES 10    /* variant 2: depth of the TMA stage ring, 2..4; 0 = as many as fit */
 #define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 

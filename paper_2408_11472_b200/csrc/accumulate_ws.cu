@@ -1,0 +1,433 @@
+// Steps A1-A7, production kernel: scatterers -> spectrum T_u[G][N] (Algorithm 1 body and
+// `rasterize`).  sm_100a, no tensor cores: a streaming scan of 28 B per scatterer with a
+// scatter-add, bounded by HBM bandwidth, instruction issue and the shared-memory atomic unit.
+//
+// Warp-specialised persistent blocks, no block-wide barrier in the steady state:
+//   * warp 0 (control): draws super-chunks of consecutive scatterers from a ticket counter, moves each chunk's
+//     seven array slices into a ring of shared-memory stages with TMA bulk copies (cp.async.bulk, completion
+//     on a `full` mbarrier), and drains finished fixed-point tiles to global memory (step A7);
+//   * warps 1..NCW (compute): wait `full`, pull their two scatterers per lane into registers, release the
+//     stage at once (`empty` mbarrier), then do geometry + amplitude (scatter_math.cuh) and add the two
+//     gate-weighted contributions into a shared-memory tile with NATIVE int32 atomics (sm_100a has no native
+//     shared fp32 add: ATOMS.CAS loops collapse under this workload's contention).
+//   * Block floating point: scatterers are processed in EPOCHS of <= 2047 scatterers.  The first warp that has
+//     something to add in an epoch fixes the epoch's Doppler window [k0, k0+W) and power-of-two scale s from
+//     its own 64 scatterers (geometric-mean amplitude * s in [2^16, 2^17)) and publishes them; everybody adds
+//     round(w c s) to an int32 tile [2][G][W+1].  A contribution outside the window or with |c| s outside
+//     [2^11, 2^20] "escapes" to an exact global fp32 reduction (rare).  <= 2047 adds of <= 2^20 per cell: no
+//     overflow.  Two tiles alternate: while the control warp drains epoch e (x 2^-e -> red.global.add.v2.f32
+//     into T), the compute warps already fill the other tile with epoch e+1.
+//   Quantisation: LSB = 1/s <= gmean * 2^-16, relative L2 error of an epoch <= 0.82 * 2^-16 = 1.3e-5 for
+//   amplitudes near their geometric mean and <= 0.82 * 2^-11 for the dimmest admitted scatterer, whose power
+//   is then 2^-10 of the typical one.
+#include <climits>
+
+#include "ptx_util.cuh"
+#include "scatter_math.cuh"
+
+namespace simk {
+
+constexpr int kWsPT = 2;          // scatterers per lane per chunk (one 8-byte shared load per array)
+constexpr int kWsMaxStages = 4;
+constexpr int kMaxEpochAdds = 2047;
+
+// epoch parameter slot (ring of 4): 8 ints
+enum { kSlState = 0, kSlK0 = 1, kSlEx = 2, kSlGmin = 3, kSlGmax = 4, kSlInts = 8 };
+enum { kStUnset = 0, kStClaimed = 1, kStReady = 2 };
+
+int acc_ws_chunk(int ncw) { return ncw * 32 * kWsPT; }
+
+size_t acc_ws_smem_bytes(int G, int W, int ncw, int stages) {
+  return (size_t)stages * 7 * acc_ws_chunk(ncw) * sizeof(float) + (size_t)2 * 2 * G * (W + 1) * sizeof(int);
+}
+
+// Scheduler state of the control warp's lane 0: the sequence of chunks of this block.
+struct Cursor {
+  unsigned long long next, end;  // next chunk start, end of the current super-chunk
+  bool done;
+};
+
+// Lane 0 of the control warp: describe the next chunk of the block's sequence in the stage's descriptor
+// (base, valid count; count 0 = end of work) and start its TMA copies.  Floats beyond the last whole group
+// of four are left to the consumers.  Returns the valid count.
+template <int CH>
+__device__ __forceinline__ unsigned produce_chunk(const AccParams& p, Cursor& c, unsigned long long n_sc,
+                                                  unsigned stage_smem, unsigned desc, unsigned bar) {
+  if (!c.done && c.next >= c.end) {
+    const unsigned long long sc = atomicAdd(&p.counters[kCtrTicket], 1u);
+    if (sc >= n_sc) {
+      c.done = true;
+    } else {
+      c.next = sc * p.superchunk;
+      c.end = (c.next + p.superchunk < p.n) ? c.next + p.superchunk : p.n;
+    }
+  }
+  unsigned nvalid = 0;
+  unsigned long long base = 0;
+  if (!c.done) {
+    base = c.next;
+    nvalid = (unsigned)((c.end - base < (unsigned long long)CH) ? c.end - base : CH);
+    c.next = base + nvalid;
+  }
+  sh::st64(desc, base);
+  sh::st(desc + 8, (int)nvalid);
+  const unsigned bytes = (nvalid & ~3u) * 4u;
+  sh::mbar_arrive_expect_tx(bar, 7u * bytes);  // release: the descriptor is visible to whoever sees the phase complete
+  if (bytes) {
+    const float* src[7] = {p.x, p.y, p.z, p.vx, p.vy, p.vz, p.s0dA};
+#pragma unroll
+    for (int a = 0; a < 7; ++a) sh::bulk_g2s(stage_smem + (unsigned)a * CH * 4u, src[a] + base, bytes, bar);
+  }
+  return nvalid;
+}
+
+// Control warp: drain the tile of epoch e (step A7) and hand it back to the compute warps.
+__device__ __forceinline__ void drain_epoch(const AccParams& p, unsigned e, unsigned tile0, unsigned tile_bytes,
+                                            unsigned plane_bytes, unsigned slot0, unsigned tdone0, unsigned tfree0,
+                                            int lane) {
+  const unsigned b = e & 1u;
+  sh::mbar_wait(tdone0 + 8u * b, (e >> 1) & 1u);  // every compute warp has finished epoch e
+  const unsigned slot = slot0 + 4u * kSlInts * (e & 3u);
+  if (sh::ld(slot + 4 * kSlState) == kStReady) {
+    const int W = p.W, N = p.N, RS = W + 1;
+    const int logW = 31 - __clz(W);
+    const int k0 = sh::ld(slot + 4 * kSlK0), ex = sh::ld(slot + 4 * kSlEx);
+    const float inv_s = __int_as_float((127 - ex) << 23);
+    const int r0 = max(sh::ld(slot + 4 * kSlGmin), 0), r1 = min(sh::ld(slot + 4 * kSlGmax) + 1, p.G - 1);
+    const int ncell = (r1 >= r0) ? (r1 - r0 + 1) << logW : 0;   // nothing fitted (all escaped): empty range
+    const unsigned tile = tile0 + b * tile_bytes;
+    for (int cc = lane; cc < ncell; cc += 32) {
+      const int r = r0 + (cc >> logW), kw = cc & (W - 1);
+      const unsigned a = tile + 4u * (unsigned)(r * RS + kw);
+      const int re = sh::ld(a), im = sh::ld(a + plane_bytes);
+      if (re | im) {
+        sh::st(a, 0);
+        sh::st(a + plane_bytes, 0);
+        atomicAdd(&p.T[(size_t)r * N + ((k0 + kw) & (N - 1))], make_float2((float)re * inv_s, (float)im * inv_s));
+      }
+    }
+    __syncwarp();
+    if (lane == 0) {
+      sh::st(slot + 4 * kSlState, kStUnset);
+      sh::st(slot + 4 * kSlGmin, INT_MAX);
+      sh::st(slot + 4 * kSlGmax, INT_MIN);
+    }
+  }
+  __syncwarp();
+  if (lane == 0) sh::mbar_arrive(tfree0 + 8u * b);  // release: zeroed tile and reset slot are visible
+}
+
+// round(v) for |v| <= 2^22 by the 1.5 * 2^23 trick (round to nearest even: unbiased), as an int
+__device__ __forceinline__ int fx_round(float a, float b) {
+  return __float_as_int(fmaf(a, b, 12582912.0f)) - 0x4B400000;
+}
+
+template <int NCW, bool FAST>
+__global__ void __launch_bounds__((NCW + 1) * 32, (NCW <= 14 ? 2 : 1)) acc_ws_kernel(AccParams p) {
+  constexpr int CH = NCW * 32 * kWsPT;
+  constexpr unsigned kStageBytes = 7u * CH * 4u;
+  constexpr unsigned kFull = 0xffffffffu;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long s_full[kWsMaxStages], s_empty[kWsMaxStages], s_tdone[2], s_tfree[2];
+  __shared__ __align__(16) unsigned s_desc[kWsMaxStages][4];
+  __shared__ int s_slot[4][kSlInts];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int S = p.stages, EC = p.epoch_chunks;
+  const int G = p.G, N = p.N, W = p.W, RS = W + 1;
+  const unsigned stage0 = sh::addr(smem_raw);
+  const unsigned tile0 = stage0 + (unsigned)S * kStageBytes;     // int [2 tiles][2 planes: re, im][G][W+1]
+  const unsigned plane_bytes = (unsigned)(G * RS) * 4u, tile_bytes = 2u * plane_bytes;
+  const unsigned full0 = sh::addr(&s_full[0]), empty0 = sh::addr(&s_empty[0]);
+  const unsigned tdone0 = sh::addr(&s_tdone[0]), tfree0 = sh::addr(&s_tfree[0]);
+  const unsigned desc0 = sh::addr(&s_desc[0][0]), slot0 = sh::addr(&s_slot[0][0]);
+
+  for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * (NCW + 1) * 32) sh::st(tile0 + a, 0);
+  if (tid < 4) {
+    sh::st(slot0 + 4u * kSlInts * tid + 4 * kSlState, kStUnset);
+    sh::st(slot0 + 4u * kSlInts * tid + 4 * kSlGmin, INT_MAX);
+    sh::st(slot0 + 4u * kSlInts * tid + 4 * kSlGmax, INT_MIN);
+  }
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      sh::mbar_init(full0 + 8u * s, 1);
+      sh::mbar_init(empty0 + 8u * s, NCW);
+    }
+    for (int b = 0; b < 2; ++b) {
+      sh::mbar_init(tdone0 + 8u * b, NCW);
+      sh::mbar_init(tfree0 + 8u * b, 1);
+    }
+    sh::mbar_fence_init();
+  }
+  __syncthreads();   // the only block-wide barrier
+
+  if (warp == 0) {
+    // ================= control warp: TMA producer + tile drain =================
+    const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
+    Cursor cursor{0, 0, false};
+    unsigned c_end = kFull;   // index of the end-of-work chunk, once known
+    for (int s = 0; s < S; ++s) {
+      if (c_end != kFull) break;
+      unsigned nv = 0;
+      if (lane == 0) nv = produce_chunk<CH>(p, cursor, n_sc, stage0 + (unsigned)s * kStageBytes, desc0 + 16u * s, full0 + 8u * s);
+      nv = __shfl_sync(kFull, nv, 0);
+      if (nv == 0) c_end = (unsigned)s;
+    }
+    unsigned stg = 0, ph = 0, ec_i = 0, e = 0;
+    for (unsigned c = 0; c < c_end; ++c) {
+      sh::mbar_wait(empty0 + 8u * stg, ph);   // every compute warp has pulled chunk c out of its stage
+      if (c_end == kFull) {
+        unsigned nv = 0;
+        if (lane == 0) nv = produce_chunk<CH>(p, cursor, n_sc, stage0 + stg * kStageBytes, desc0 + 16u * stg, full0 + 8u * stg);
+        nv = __shfl_sync(kFull, nv, 0);
+        if (nv == 0) c_end = c + (unsigned)S;
+      }
+      if (++ec_i == (unsigned)EC) {
+        drain_epoch(p, e, tile0, tile_bytes, plane_bytes, slot0, tdone0, tfree0, lane);
+        ec_i = 0;
+        ++e;
+      }
+      if (++stg == (unsigned)S) { stg = 0; ph ^= 1u; }
+    }
+    if (ec_i != 0) drain_epoch(p, e, tile0, tile_bytes, plane_bytes, slot0, tdone0, tfree0, lane);
+    return;
+  }
+
+  // ================= compute warps =================
+  const unsigned e0 = (unsigned)((warp - 1) * 32 + lane) * kWsPT;   // this lane's first scatterer in a chunk
+  const int halfN = N >> 1;
+  unsigned stg = 0, ph = 0, ec_i = 0, e = 0;
+  int my_epoch = -1;         // epoch whose parameters this warp holds
+  int k0 = 0, lo_bits = 0;
+  float s = 0.0f;
+  unsigned tile_b = tile0;
+  int gmin = INT_MAX, gmax = INT_MIN;
+  unsigned escapes = 0, fallbacks = 0;
+
+  for (;;) {
+    if (ec_i == 0 && e >= 2) sh::mbar_wait(tfree0 + 8u * (e & 1u), ((e >> 1) - 1u) & 1u);  // tile of epoch e-2 drained
+    sh::mbar_wait(full0 + 8u * stg, ph);
+    const unsigned desc = desc0 + 16u * stg;
+    const unsigned nvalid = (unsigned)sh::ld(desc + 8);
+    if (nvalid == 0) break;  // block-uniform: end of work
+
+    // ---- step A1: this lane's two scatterers, shared-memory stage -> registers; stage released at once ----
+    float2 x, y, z, vx, vy, vz, s0;
+    if (e0 + kWsPT <= (nvalid & ~3u)) {
+      const unsigned a = stage0 + stg * kStageBytes + e0 * 4u;
+      x = sh::ldf2(a + 0u * CH * 4u);
+      y = sh::ldf2(a + 1u * CH * 4u);
+      z = sh::ldf2(a + 2u * CH * 4u);
+      vx = sh::ldf2(a + 3u * CH * 4u);
+      vy = sh::ldf2(a + 4u * CH * 4u);
+      vz = sh::ldf2(a + 5u * CH * 4u);
+      s0 = sh::ldf2(a + 6u * CH * 4u);
+    } else {  // ragged end of the input: not covered by the 16-byte bulk copies; s0dA = 0 contributes nothing
+      const unsigned long long base = sh::ld64(desc);
+      const bool v0 = e0 < nvalid, v1 = e0 + 1 < nvalid;
+      const unsigned long long i0 = base + e0, i1 = i0 + 1;
+      x = make_float2(v0 ? p.x[i0] : 0.0f, v1 ? p.x[i1] : 0.0f);
+      y = make_float2(v0 ? p.y[i0] : 0.0f, v1 ? p.y[i1] : 0.0f);
+      z = make_float2(v0 ? p.z[i0] : 0.0f, v1 ? p.z[i1] : 0.0f);
+      vx = make_float2(v0 ? p.vx[i0] : 0.0f, v1 ? p.vx[i1] : 0.0f);
+      vy = make_float2(v0 ? p.vy[i0] : 0.0f, v1 ? p.vy[i1] : 0.0f);
+      vz = make_float2(v0 ? p.vz[i0] : 0.0f, v1 ? p.vz[i1] : 0.0f);
+      s0 = make_float2(v0 ? p.s0dA[i0] : 0.0f, v1 ? p.s0dA[i1] : 0.0f);
+    }
+    __syncwarp();
+    if (lane == 0) sh::mbar_arrive(empty0 + 8u * stg);
+
+    // ---- steps A2-A5 ----
+    bool ok0 = s0.x > 0.0f, ok1 = s0.y > 0.0f;   // s0dA <= 0 or NaN: dead
+    const Pre q0 = pre_part<FAST>(p, x.x, y.x, z.x, ok0);
+    const Pre q1 = pre_part<FAST>(p, x.y, y.y, z.y, ok1);
+    if (__any_sync(kFull, ok0 | ok1)) {  // warp-uniform: skip warps that are entirely dark
+      Idx i0, i1;
+      ok0 = index_part<FAST>(p, q0, vx.x, vy.x, vz.x, ok0, i0, fallbacks);
+      ok1 = index_part<FAST>(p, q1, vx.y, vy.y, vz.y, ok1, i1, fallbacks);
+      float A0, A1;
+      const float2 c0 = amplitude(p, x.x, y.x, z.x, i0.gfx, i0.fr, s0.x, A0);
+      const float2 c1 = amplitude(p, x.y, y.y, z.y, i1.gfx, i1.fr, s0.y, A1);
+      const int ab0 = __float_as_int(A0), ab1 = __float_as_int(A1);
+      const unsigned okm = __ballot_sync(kFull, ok0 | ok1);
+      if (okm) {
+        // ---- epoch parameters: the first warp with something to add decides them ----
+        if (my_epoch != (int)e) {
+          const unsigned slot = slot0 + 4u * kSlInts * (e & 3u);
+          int st = 0;
+          if (lane == 0) {
+            st = sh::ld_acquire(slot + 4 * kSlState);
+            if (st != kStReady) st = sh::cas(slot + 4 * kSlState, kStUnset, kStClaimed);
+          }
+          st = __shfl_sync(kFull, st, 0);
+          if (st == kStUnset) {  // this warp won the claim: window and scale from its own scatterers
+            const int kk = ok0 ? i0.k : i1.k;
+            const int kref = __shfl_sync(kFull, kk, __ffs(okm) - 1) & (N - 1);
+            const int d0 = ((i0.k - kref + halfN) & (N - 1)) - halfN;   // signed circular bin offsets
+            const int d1 = ((i1.k - kref + halfN) & (N - 1)) - halfN;
+            int dmin = min(ok0 ? d0 : INT_MAX, ok1 ? d1 : INT_MAX);
+            int dmax = max(ok0 ? d0 : INT_MIN, ok1 ? d1 : INT_MIN);
+            int cnt = (ok0 ? 1 : 0) + (ok1 ? 1 : 0);
+            int slog = (ok0 ? (ab0 >> 16) : 0) + (ok1 ? (ab1 >> 16) : 0);   // log2 amplitude, 2^-7 units
+            dmin = __reduce_min_sync(kFull, dmin);
+            dmax = __reduce_max_sync(kFull, dmax);
+            cnt = __reduce_add_sync(kFull, cnt);
+            slog = __reduce_add_sync(kFull, slog);
+            if (lane == 0) {
+              const int centre = (dmax - dmin < W) ? kref + ((dmin + dmax + 1) >> 1) : kref;
+              const int E = (slog / cnt) >> 7;                 // biased exponent of the geometric mean
+              const int ex = max(-100, min(120, 16 - (E - 127)));   // gmean * 2^ex in [2^16, 2^17)
+              sh::st(slot + 4 * kSlK0, (centre - (W >> 1)) & (N - 1));
+              sh::st(slot + 4 * kSlEx, ex);
+              sh::st_release(slot + 4 * kSlState, kStReady);
+            }
+            __syncwarp();
+          } else if (st == kStClaimed) {
+            while (sh::ld_acquire(slot + 4 * kSlState) != kStReady) {
+            }
+          }
+          k0 = sh::ld(slot + 4 * kSlK0);
+          const int ex = sh::ld(slot + 4 * kSlEx);
+          s = __int_as_float((ex + 127) << 23);
+          lo_bits = (11 - ex + 127) << 23;                    // bits of 2^11 / s
+          tile_b = tile0 + (e & 1u) * tile_bytes;
+          my_epoch = (int)e;
+        }
+        // ---- step A6: native int32 shared-memory atomics; what does not fit escapes to global fp32 ----
+        bool esc0, esc1;
+        {
+          const unsigned kw = (unsigned)(i0.k - k0) & (unsigned)(N - 1);
+          const bool fits = ok0 && kw < (unsigned)W && (unsigned)(ab0 - lo_bits) <= (9u << 23);
+          const float w1s = i0.w1 * s, w0s = s - w1s;
+          const unsigned a0 = tile_b + 4u * (unsigned)(i0.g0 * RS + (int)kw);
+          if (fits && i0.g0 >= 0) {
+            sh::red_add(a0, fx_round(c0.x, w0s));
+            sh::red_add(a0 + plane_bytes, fx_round(c0.y, w0s));
+          }
+          if (fits && i0.g0 + 1 < G) {
+            const unsigned a1 = a0 + 4u * (unsigned)RS;
+            sh::red_add(a1, fx_round(c0.x, w1s));
+            sh::red_add(a1 + plane_bytes, fx_round(c0.y, w1s));
+          }
+          gmin = min(gmin, fits ? i0.g0 : INT_MAX);
+          gmax = max(gmax, fits ? i0.g0 : INT_MIN);
+          esc0 = ok0 && !fits;
+        }
+        {
+          const unsigned kw = (unsigned)(i1.k - k0) & (unsigned)(N - 1);
+          const bool fits = ok1 && kw < (unsigned)W && (unsigned)(ab1 - lo_bits) <= (9u << 23);
+          const float w1s = i1.w1 * s, w0s = s - w1s;
+          const unsigned a0 = tile_b + 4u * (unsigned)(i1.g0 * RS + (int)kw);
+          if (fits && i1.g0 >= 0) {
+            sh::red_add(a0, fx_round(c1.x, w0s));
+            sh::red_add(a0 + plane_bytes, fx_round(c1.y, w0s));
+          }
+          if (fits && i1.g0 + 1 < G) {
+            const unsigned a1 = a0 + 4u * (unsigned)RS;
+            sh::red_add(a1, fx_round(c1.x, w1s));
+            sh::red_add(a1 + plane_bytes, fx_round(c1.y, w1s));
+          }
+          gmin = min(gmin, fits ? i1.g0 : INT_MAX);
+          gmax = max(gmax, fits ? i1.g0 : INT_MIN);
+          esc1 = ok1 && !fits;
+        }
+        if (__any_sync(kFull, esc0 | esc1)) {  // rare
+          if (esc0) {
+            const int k = i0.k & (N - 1);
+            const float w0 = 1.0f - i0.w1;
+            if (i0.g0 >= 0) atomicAdd(&p.T[(size_t)i0.g0 * N + k], make_float2(w0 * c0.x, w0 * c0.y));
+            if (i0.g0 + 1 < G) atomicAdd(&p.T[(size_t)(i0.g0 + 1) * N + k], make_float2(i0.w1 * c0.x, i0.w1 * c0.y));
+            ++escapes;
+          }
+          if (esc1) {
+            const int k = i1.k & (N - 1);
+            const float w0 = 1.0f - i1.w1;
+            if (i1.g0 >= 0) atomicAdd(&p.T[(size_t)i1.g0 * N + k], make_float2(w0 * c1.x, w0 * c1.y));
+            if (i1.g0 + 1 < G) atomicAdd(&p.T[(size_t)(i1.g0 + 1) * N + k], make_float2(i1.w1 * c1.x, i1.w1 * c1.y));
+            ++escapes;
+          }
+        }
+      }
+    }
+
+    // ---- end of an epoch: row range of what this warp added, then hand the tile to the control warp ----
+    if (++ec_i == (unsigned)EC) {
+      if (my_epoch == (int)e) {
+        gmin = __reduce_min_sync(kFull, gmin);
+        gmax = __reduce_max_sync(kFull, gmax);
+        if (lane == 0 && gmin <= gmax) {
+          sh::red_min(slot0 + 4u * kSlInts * (e & 3u) + 4 * kSlGmin, gmin);
+          sh::red_max(slot0 + 4u * kSlInts * (e & 3u) + 4 * kSlGmax, gmax);
+        }
+        gmin = INT_MAX;
+        gmax = INT_MIN;
+      }
+      __syncwarp();
+      if (lane == 0) sh::mbar_arrive(tdone0 + 8u * (e & 1u));
+      ec_i = 0;
+      ++e;
+    }
+    if (++stg == (unsigned)S) { stg = 0; ph ^= 1u; }
+  }
+  if (ec_i != 0) {  // the input ended inside an epoch
+    if (my_epoch == (int)e) {
+      gmin = __reduce_min_sync(kFull, gmin);
+      gmax = __reduce_max_sync(kFull, gmax);
+      if (lane == 0 && gmin <= gmax) {
+        sh::red_min(slot0 + 4u * kSlInts * (e & 3u) + 4 * kSlGmin, gmin);
+        sh::red_max(slot0 + 4u * kSlInts * (e & 3u) + 4 * kSlGmax, gmax);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) sh::mbar_arrive(tdone0 + 8u * (e & 1u));
+  }
+  if (escapes) atomicAdd(&p.counters[kCtrEscape], escapes);
+  if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Launchers
+// ---------------------------------------------------------------------------------------------
+typedef void (*WsKernel)(AccParams);
+
+static WsKernel ws_kernel(int ncw, bool fast) {
+  switch (ncw) {
+    case 30: return fast ? acc_ws_kernel<30, true> : acc_ws_kernel<30, false>;
+    case 22: return fast ? acc_ws_kernel<22, true> : acc_ws_kernel<22, false>;
+    case 14: return fast ? acc_ws_kernel<14, true> : acc_ws_kernel<14, false>;
+    case 7: return fast ? acc_ws_kernel<7, true> : acc_ws_kernel<7, false>;
+    default: return nullptr;
+  }
+}
+
+cudaError_t acc_ws_blocks_per_sm(int G, int W, int ncw, int stages, int* blocks) {
+  const size_t smem = acc_ws_smem_bytes(G, W, ncw, stages);
+  *blocks = 1 << 30;
+  for (int fast = 0; fast < 2; ++fast) {
+    WsKernel k = ws_kernel(ncw, fast != 0);
+    if (!k) return cudaErrorInvalidValue;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int b = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k, (ncw + 1) * 32, smem);
+    if (e != cudaSuccess) return e;
+    if (b < *blocks) *blocks = b;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t launch_accumulate_ws(const AccParams& p, int ncw, int blocks, cudaStream_t st, int* launches) {
+  if (p.n == 0) return cudaSuccess;
+  WsKernel k = ws_kernel(ncw, p.index_path && p.fast_ok);
+  if (!k) return cudaErrorInvalidValue;
+  const size_t smem = acc_ws_smem_bytes(p.G, p.W, ncw, p.stages);
+  cudaError_t e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
+  if (e != cudaSuccess) return e;
+  const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
+  const int grid = (int)(n_sc < (unsigned long long)blocks ? n_sc : (unsigned long long)blocks);
+  k<<<grid, (ncw + 1) * 32, smem, st>>>(p);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+}  // namespace simk

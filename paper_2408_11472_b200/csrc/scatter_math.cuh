@@ -1,0 +1,161 @@
+// Steps A2-A5 of one scatterer: geometry -> (gate, Doppler bin, gate weight, phase) ->
+// complex amplitude.  Paper: `scatterers_range`, `scatterers_complex_amplitudes`, the coordinates of
+// `rasterize`.  Used by every accumulation kernel and by the index-only kernel.
+#pragma once
+#include "sim_internal.h"
+
+namespace simk {
+
+// 1.5 * 2^(52 - kFracBits): adding it to v (|v| < 2^11) leaves floor/round(v * 2^20) in the low word.
+constexpr double kMagicFx = 6442450944.0;        // 1.5 * 2^32
+constexpr double kMagicFxHalf = 6442450944.5;    // the same + 0.5 (nearest-bin rule, ties up)
+constexpr double kMagicPhase = 402653184.0;      // 1.5 * 2^28: low word = round(q * 2^24)
+constexpr int kFxOne = 1 << kFracBits;
+
+// What the index part of one scatterer yields.
+struct Idx {
+  int g0;      // gate of the lower half, in [-1, G-1]
+  int k;       // Doppler bin; congruent to the bin mod N (not yet wrapped on the fast path)
+  float w1;    // weight of gate g0+1 (gate g0 gets 1 - w1)
+  float fr;    // frac(2R/lambda) mapped to [-0.5, 0.5) cycles
+  float gfx;   // gf * 2^kFracBits as a float (for 1/R^2)
+};
+
+// frac(q) of q cycles as a float in [-0.5, 0.5): round(q * 2^24) sits in the low word after the magic add
+__device__ __forceinline__ float cycles_fraction(double q) {
+  const int lo = __double2loint(__dadd_rn(q, kMagicPhase));
+  return (float)(int)((unsigned)lo << 8) * 2.3283064365386963e-10f;  // * 2^-32
+}
+
+// ---------------------------------------------------------------------------------------------
+// CANONICAL fp64 INDEX SEQUENCE of DESIGN.md, from dx, dy, dz.  Explicit round-to-nearest
+// intrinsics: nvcc must not contract a*b+c differently from the definition.  Out of line (the fast
+// path calls it only inside the guard band) and fed by value.
+// Returns (g0, k wrapped, bits of w1, bits of fr); g0 = SIM_GATE_NONE when the scatterer is dropped.
+// ---------------------------------------------------------------------------------------------
+struct CanonConsts {
+  double rg0, inv_dR, cD, two_over_lambda, fr0, svx, svy, svz;
+  int G, N;
+};
+
+static __device__ __noinline__ int4 canonical_tail(CanonConsts c, double dx, double dy, double dz, float vxf,
+                                                   float vyf, float vzf) {
+  const int4 dropped = make_int4(SIM_GATE_NONE, -1, 0, 0);
+  const double R2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+  const double R = __dsqrt_rn(R2);
+  const double delta = __dsub_rn(R, c.rg0);
+  const double gf = __dmul_rn(delta, c.inv_dR);
+  if (!(gf >= -1.0 && gf < (double)c.G)) return dropped;  // touches no gate (NaN lands here too)
+  const double g0d = floor(gf);
+  const double dvx = __dsub_rn((double)vxf, c.svx);
+  const double dvy = __dsub_rn((double)vyf, c.svy);
+  const double dvz = __dsub_rn((double)vzf, c.svz);
+  const double rdot = __ddiv_rn(__fma_rn(dvz, dz, __fma_rn(dvy, dy, __dmul_rn(dvx, dx))), R);
+  const double kf = __dmul_rn(rdot, c.cD);
+  if (!(fabs(kf) < 1073741824.0)) return dropped;
+  const double kk = floor(__dadd_rn(kf, 0.5));
+  // N is a power of two: two's-complement AND is the mathematical mod
+  const double q = __fma_rn(delta, c.two_over_lambda, c.fr0);  // only the fraction of 2R/lambda matters
+  return make_int4((int)g0d, ((int)kk) & (c.N - 1), __float_as_int((float)__dsub_rn(gf, g0d)),
+                   __float_as_int(cycles_fraction(q)));
+}
+
+__device__ __forceinline__ bool canonical(const AccParams& p, double dx, double dy, double dz, float vxf,
+                                          float vyf, float vzf, Idx& o) {
+  CanonConsts c;
+  c.rg0 = p.rg0; c.inv_dR = p.inv_dR; c.cD = p.cD; c.two_over_lambda = p.two_over_lambda; c.fr0 = p.fr0;
+  c.svx = p.svx; c.svy = p.svy; c.svz = p.svz; c.G = p.G; c.N = p.N;
+  const int4 r = canonical_tail(c, dx, dy, dz, vxf, vyf, vzf);
+  if (r.x == SIM_GATE_NONE) return false;
+  o.g0 = r.x;
+  o.k = r.y;
+  o.w1 = __int_as_float(r.z);
+  o.fr = __int_as_float(r.w);
+  o.gfx = ((float)r.x + o.w1) * (float)kFxOne;
+  return true;
+}
+
+// Steps A2-A4 in two parts, so that a warp whose scatterers all miss the window can stop after the first.
+//   FAST = false: the canonical sequence for every scatterer.
+//   FAST = true:  everything is a short polynomial in u = R^2 - rg0^2 (no sqrt, no divide):
+//       gf = (R - rg0)/dR = u (g1 + u (g2 + u g3)),   kf = num cD / R = num (j0 + u (j1 + u j2)),
+//     gate and bin are read from 2^-20 fixed point; whenever a coordinate lies within `guard` of an
+//     integer boundary the canonical sequence decides (bit-exact indices).
+struct Pre {
+  double dx, dy, dz, u;
+};
+
+// Offsets from the satellite and the window pre-test.  `live` in: the scatterer is a candidate (s0dA > 0);
+// out: it may land in the gate window.
+template <bool FAST>
+__device__ __forceinline__ Pre pre_part(const AccParams& p, float xf, float yf, float zf, bool& live) {
+  Pre q;
+  q.dx = __dsub_rn((double)xf, p.sx);
+  q.dy = __dsub_rn((double)yf, p.sy);
+  q.dz = __dsub_rn((double)zf, p.sz);
+  q.u = 0.0;
+  if (FAST) {
+    // the three squares cancel against -rg0^2; every rounding is <= ulp(rg0^2) ~ 1e-4 m^2 (<< guard)
+    q.u = fma(q.dz, q.dz, fma(q.dy, q.dy, fma(q.dx, q.dx, p.neg_rg0sq)));
+    live = live && (q.u >= p.uw_lo) && (q.u <= p.uw_hi);   // false: certainly outside the window (or NaN)
+  }
+  return q;
+}
+
+// Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.
+template <bool FAST>
+__device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
+                                           bool live, Idx& o, unsigned& fallbacks) {
+  if (!FAST) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+  const double u = q.u;
+  const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
+  const int gfx = __double2loint(__dadd_rd(gf, kMagicFx));            // floor(gf * 2^20)
+  const int gfrac = gfx & (kFxOne - 1);
+  const double dvx = (double)vxf - p.svx, dvy = (double)vyf - p.svy, dvz = (double)vzf - p.svz;
+  const double num = fma(dvz, q.dz, fma(dvy, q.dy, dvx * q.dx));
+  const double kf = num * fma(u, fma(u, p.j2, p.j1), p.j0);
+  const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));        // floor((kf + 0.5) * 2^20)
+  const int kfrac = kfx & (kFxOne - 1);
+  const unsigned span = (unsigned)(kFxOne - 2 * p.guard);
+  const bool near = ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - p.guard) >= span) |
+                    !(fabs(kf) < 1024.0);
+  if (live && near) {  // rare: a coordinate sits in the guard band
+    ++fallbacks;
+    return canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+  }
+  o.g0 = gfx >> kFracBits;
+  o.k = kfx >> kFracBits;
+  o.w1 = (float)gfrac * p.w_scale;
+  o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
+  o.gfx = (float)gfx;
+  return live;
+}
+
+__device__ __forceinline__ float sqrt_approx(float v) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+__device__ __forceinline__ float ex2_approx(float v) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+
+// Step A5: sqrt(s0dA) G(theta) / R^2 exp(-i 2 pi fr), all fp32.  Returns |c| in A.
+//   1/R^2 from the gate coordinate; sin^2(theta) = ((d.e1)^2 + (d.e2)^2) / R^2 with (e1, e2, boresight)
+//   orthonormal; offsets d from the satellite in fp32 (hi + lo split only where it matters: z).
+__device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float yf, float zf, float gfx,
+                                            float fr, float s0dA, float& A) {
+  const float dx = xf - p.sxh, dy = yf - p.syh, dz = (zf - p.szh) - p.szl;
+  const float inv_R2 = fmaf(gfx, fmaf(gfx, p.a2, p.a1), p.a0);
+  const float p1 = fmaf(dz, p.e1z, fmaf(dy, p.e1y, dx * p.e1x));
+  const float p2 = fmaf(dz, p.e2z, fmaf(dy, p.e2y, dx * p.e2x));
+  const float t = fmaf(p2, p2, p1 * p1);
+  A = sqrt_approx(s0dA) * ex2_approx(t * (inv_R2 * p.neg_alpha_log2e)) * inv_R2;
+  float sn, cs;
+  __sincosf(6.283185307179586f * fr, &sn, &cs);
+  return make_float2(A * cs, -A * sn);
+}
+
+}  // namespace simk

@@ -80,6 +80,9 @@ struct sim_handle {
   int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard, opt_per_thread, opt_min_blocks;
   int64_t opt_superchunk;
   int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
+  int opt_ncw, opt_stages;          // warp-specialised kernel: compute warps per block, TMA ring depth (0 = auto)
+  int ws_W, ws_stages, ws_blocks_per_sm;
+  size_t smem_per_sm;
   // stats
   uint64_t launches, scatterers_seen;
   std::string err;
@@ -173,6 +176,25 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
   const double guard_k = p.guard / (double)(1 << kFracBits);
   const bool phase_ok = (G + 2) * dR * c < 134217728.0;   // 2^27: the magic-number fraction needs |q| < 2^28
   if (guard_m >= 4.0 * err_m && guard_k >= 4.0 * err_k && phase_ok && G + 2 < 2048) p.fast_ok = 1;
+  {  // polynomial index path of the warp-specialised kernel (scatter_math.cuh), x = u / rg0^2 <= ~2 emax
+    const double r2 = rg0 * rg0, gd = p.guard / (double)(1 << kFracBits);
+    p.neg_rg0sq = -r2;
+    p.g1 = 1.0 / (2.0 * rg0 * dR);
+    p.g2 = -1.0 / (8.0 * rg0 * r2 * dR);
+    p.g3 = 1.0 / (16.0 * rg0 * r2 * r2 * dR);
+    p.j0 = p.cD / rg0;
+    p.j1 = -p.cD / (2.0 * rg0 * r2);
+    p.j2 = 3.0 * p.cD / (8.0 * rg0 * r2 * r2);
+    p.cq = dR * c;
+    const double mg = 0.5 * gd;                                   // window margin, gates (half a guard band)
+    const double wl = -dR * (1.0 + mg), wh = dR * (G + mg);
+    p.uw_lo = wl * (2.0 * rg0 + wl);
+    p.uw_hi = wh * (2.0 * rg0 + wh);
+    const double x = 2.2 * emax;
+    const double eg = 0.04 * x * x * x * x * rg0 / dR + 4.0 * std::ldexp(r2, -52) / (2.0 * rg0 * dR) + 1e-13 * (G + 2);
+    const double ek = 1024.0 * (0.32 * x * x * x + 1e-14);
+    if (!(gd >= 4.0 * eg && gd >= 4.0 * ek && phase_ok && G + 2 < 2048)) p.fast_ok = 0;
+  }
   // fp32 pre-test: |u_f32 - u| <= 2^-21 R^2 (three squares, two sums, the split satellite position and
   // rg0^2 each rounded to 2^-24); the margin is twice that at the far edge of the window
   const double margin_u = std::ldexp(rmax * rmax, -20);
@@ -182,7 +204,9 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
 }
 
 int acc_blocks(const sim_handle* h) {
-  return h->opt_blocks > 0 ? h->opt_blocks : h->sm_count * (h->tile_blocks_per_sm > 0 ? h->tile_blocks_per_sm : 1);
+  if (h->opt_blocks > 0) return h->opt_blocks;
+  const int per_sm = h->opt_variant == 2 ? h->ws_blocks_per_sm : h->tile_blocks_per_sm;
+  return h->sm_count * (per_sm > 0 ? per_sm : 1);
 }
 
 // (Re)chooses the window width and the resident blocks per SM; cheap, called when an option changes.
@@ -191,6 +215,30 @@ cudaError_t plan_tile(sim_handle* h) {
   int b = 1;
   cudaError_t e = acc_tile_blocks_per_sm(h->cfg.n_gates, h->tile_W, h->opt_per_thread, h->opt_min_blocks, &b);
   h->tile_blocks_per_sm = b > 0 ? b : 1;
+  return e;
+}
+
+// Warp-specialised kernel: window width, ring depth and resident blocks per SM for the shared memory there is.
+cudaError_t plan_ws(sim_handle* h) {
+  const int G = h->cfg.n_gates, N = h->cfg.n_doppler, ncw = h->opt_ncw;
+  const int target = ncw <= 7 ? 4 : (ncw <= 14 ? 2 : 1);            // blocks per SM the register budget allows
+  size_t budget = h->smem_per_sm / target;
+  budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
+  if (budget > h->smem_optin - 1024) budget = h->smem_optin - 1024;
+  const size_t stage = acc_ws_smem_bytes(0, 0, ncw, 1);
+  int w = h->opt_window > 0 ? h->opt_window : 16;
+  if (w > N) w = N;
+  while (w > 1 && acc_ws_smem_bytes(G, w, ncw, 2) > budget) w >>= 1;
+  const size_t tiles = acc_ws_smem_bytes(G, w, ncw, 0);
+  int st = tiles + 2 * stage <= budget ? (int)((budget - tiles) / stage) : 2;
+  if (st > 4) st = 4;
+  if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
+  if (st < 2) st = 2;
+  h->ws_W = w;
+  h->ws_stages = st;
+  int b = 1;
+  cudaError_t e = acc_ws_blocks_per_sm(G, w, ncw, st, &b);
+  h->ws_blocks_per_sm = b > 0 ? b : 1;
   return e;
 }
 
@@ -219,6 +267,25 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.dR_f = (float)h->cfg.gate_spacing_m;
   p.inv_rg0_f = (float)(1.0 / sat->range_gate0_m);
   p.inv_rg0sq_f = (float)(1.0 / (sat->range_gate0_m * sat->range_gate0_m));
+  {  // orthonormal basis (e1, e2) of the plane normal to the boresight: sin^2 = ((d.e1)^2 + (d.e2)^2) / R^2
+    const double b[3] = {sat->boresight[0] / bn, sat->boresight[1] / bn, sat->boresight[2] / bn};
+    int ax = 0;
+    if (std::fabs(b[1]) < std::fabs(b[ax])) ax = 1;
+    if (std::fabs(b[2]) < std::fabs(b[ax])) ax = 2;
+    double a[3] = {0, 0, 0};
+    a[ax] = 1.0;
+    double e1[3] = {b[1] * a[2] - b[2] * a[1], b[2] * a[0] - b[0] * a[2], b[0] * a[1] - b[1] * a[0]};
+    const double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    for (double& v : e1) v /= n1;
+    const double e2[3] = {b[1] * e1[2] - b[2] * e1[1], b[2] * e1[0] - b[0] * e1[2], b[0] * e1[1] - b[1] * e1[0]};
+    p.e1x = (float)e1[0]; p.e1y = (float)e1[1]; p.e1z = (float)e1[2];
+    p.e2x = (float)e2[0]; p.e2y = (float)e2[1]; p.e2z = (float)e2[2];
+    const double rg0 = sat->range_gate0_m, dRf = h->cfg.gate_spacing_m / (double)(1 << kFracBits);
+    p.a0 = (float)(1.0 / (rg0 * rg0));
+    p.a1 = (float)(-2.0 * dRf / (rg0 * rg0 * rg0));
+    p.a2 = (float)(3.0 * dRf * dRf / (rg0 * rg0 * rg0 * rg0));
+    p.w_scale = (float)(1.0 / (double)(1 << kFracBits));
+  }
   p.G = h->cfg.n_gates;
   p.N = h->cfg.n_doppler;
   p.T = T;
@@ -231,7 +298,15 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
     sc = 65536;
     while (sc > (unsigned long long)kAccChunk && s->n / sc < (unsigned long long)blocks * 8) sc >>= 1;
   }
-  sc = (sc + kAccChunk - 1) / kAccChunk * kAccChunk;
+  unsigned long long unit = kAccChunk;
+  if (h->opt_variant == 2) {
+    const int ch = acc_ws_chunk(h->opt_ncw);
+    p.W = h->ws_W;
+    p.stages = h->ws_stages;
+    p.epoch_chunks = 2047 / ch > 0 ? 2047 / ch : 1;
+    unit = (unsigned long long)ch * p.epoch_chunks;     // super-chunk = whole epochs: a jump never splits one
+  }
+  sc = (sc + unit - 1) / unit * unit;
   p.superchunk = sc;
   p.index_path = h->opt_index_path;
   return p;
@@ -241,7 +316,9 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
   AccParams p = make_acc_params(h, d_scat, sat, T);
   const int blocks = acc_blocks(h);
   int l = 0;
-  cudaError_t e = launch_accumulate(p, h->opt_variant, h->opt_per_thread, h->opt_min_blocks, blocks, h->stream, &l);
+  cudaError_t e = h->opt_variant == 2
+                      ? launch_accumulate_ws(p, h->opt_ncw, blocks, h->stream, &l)
+                      : launch_accumulate(p, h->opt_variant, h->opt_per_thread, h->opt_min_blocks, blocks, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
@@ -343,7 +420,9 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->stage_used[0] = h->stage_used[1] = false;
   h->n_updates = 0;
   h->pulses_emitted = 0;
-  h->opt_variant = 1;
+  h->opt_variant = 2;
+  h->opt_ncw = 14;
+  h->opt_stages = 0;
   h->opt_blocks = 0;
   h->opt_window = 0;
   h->opt_index_path = 1;
@@ -370,7 +449,11 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
       cudaEventCreateWithFlags(&h->ev_consumed[b], cudaEventDisableTiming);
     }
   }
+  e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, cfg->device);
+  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem per SM)"); }
+  h->smem_per_sm = (size_t)v;
   e = plan_tile(h);
+  if (e == cudaSuccess) e = plan_ws(h);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters)"); }
@@ -523,7 +606,7 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
   if (value < 0) return fail(h, SIM_ERR_INVALID_ARG, "option value < 0");
   switch (option) {
     case SIM_OPT_ACC_VARIANT:
-      if (value > 1) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
+      if (value > 2) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
       h->opt_variant = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_BLOCKS:
@@ -538,6 +621,7 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
       h->opt_window = (int)value;
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;
     case SIM_OPT_ACC_PER_THREAD:
       if (value != 2 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "scatterers per thread must be 2 or 4");
@@ -548,6 +632,16 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       if (value < 2 || value > 4) return fail(h, SIM_ERR_INVALID_ARG, "register budget: 2..4 blocks per SM");
       h->opt_min_blocks = (int)value;
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      return SIM_OK;
+    case SIM_OPT_ACC_WARPS:
+      if (value != 7 && value != 14 && value != 22 && value != 30) return fail(h, SIM_ERR_INVALID_ARG, "compute warps per block: 7, 14, 22 or 30");
+      h->opt_ncw = (int)value;
+      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      return SIM_OK;
+    case SIM_OPT_ACC_STAGES:
+      if (value > 4 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..4");
+      h->opt_stages = (int)value;
+      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;
     case SIM_OPT_GUARD_LSB:
       if (value < 1 || value > (1 << (kFracBits - 2))) return fail(h, SIM_ERR_INVALID_ARG, "guard must be in 1..2^18");

@@ -55,6 +55,16 @@ struct AccParams {
   unsigned long long superchunk; // scatterers per scheduling unit (multiple of kAccChunk)
   int W;                  // Doppler bins of the shared-memory window (power of two, <= N)
   int index_path;         // 0 canonical everywhere, 1 fast path + guard band
+  // ---- warp-specialised kernel (accumulate_ws.cu): polynomial index path in u = R^2 - rg0^2 ----
+  double neg_rg0sq;       // -(rg0 * rg0), rounded once
+  double uw_lo, uw_hi;    // u outside [uw_lo, uw_hi]: outside the gate window by more than half a guard band
+  double g1, g2, g3;      // gf = u (g1 + u (g2 + u g3))            = (R - rg0) / dR
+  double j0, j1, j2;      // kf = num (j0 + u (j1 + u j2))          = num cD / R
+  double cq;              // dR * 2 / lambda: cycles of phase per gate
+  float e1x, e1y, e1z, e2x, e2y, e2z;  // orthonormal basis of the plane normal to the boresight
+  float a0, a1, a2;       // 1/R^2 = a0 + gfx (a1 + gfx a2), gfx = gf * 2^kFracBits
+  float w_scale;          // 2^-kFracBits
+  int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
 };
 
 struct SynParams {
@@ -74,6 +84,11 @@ struct SynParams {
 
 cudaError_t launch_accumulate(const AccParams& p, int variant, int per_thread, int min_blocks, int blocks,
                               cudaStream_t st, int* launches);
+// warp-specialised kernel: ncw compute warps + 1 control warp per block
+size_t acc_ws_smem_bytes(int G, int W, int ncw, int stages);
+cudaError_t acc_ws_blocks_per_sm(int G, int W, int ncw, int stages, int* blocks);
+cudaError_t launch_accumulate_ws(const AccParams& p, int ncw, int blocks, cudaStream_t st, int* launches);
+int acc_ws_chunk(int ncw);
 cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
                            int* launches);
 size_t acc_tile_smem_bytes(int G, int W, int per_thread);
