@@ -335,7 +335,7 @@ def main():
 
     peak, peak_src = measured_peak()
     achieved = BYTES_PER_SCATTERER * n_local / (acc_ms_mean * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "acc_ws_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "acc_ws3_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": committed_traffic(wl.name), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": BYTES_PER_SCATTERER * n_local, "launch_ms": acc_ms_mean,
                 "frac_of_8TBs_nominal": achieved / 8000.0}

@@ -155,7 +155,9 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 
 /* Tuning knobs (benchmarks and tests; defaults are chosen by the library). */
 #define SIM_OPT_ACC_VARIANT 1   /* 0 = reference kernel (global atomics), 1 = barrier-synchronised tile kernel,
-                                   2 = warp-specialised tile kernel (default) */
+                                   2 = warp-specialised tile kernel (control warp + compute warps),
+                                   3 = producer warp + drain warp + compute warps, long epochs (default).
+                                   Selecting a variant resets warps / per-lane / epoch options to its defaults */
 #define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto */
 #define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit; 0 = auto */
 #define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto */
@@ -164,6 +166,11 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_MIN_BLOCKS 8 /* register budget of the tile kernel: compiled for 2..4 resident blocks per SM */
 #define SIM_OPT_ACC_WARPS 9      /* variant 2: compute warps per block: 7, 14 (default), 22 or 30 */
 #define SIM_OPT_ACC_STAGES 10    /* variant 2: depth of the TMA stage ring, 2..4; 0 = as many as fit */
+#define SIM_OPT_ACC_PER_LANE 11  /* variant 3: scatterers per lane per chunk: 2 or 4 */
+#define SIM_OPT_ACC_EPOCH 12     /* variants 2, 3: scatterers per fixed-point epoch, 64..2047 (default 2047) */
+#define SIM_OPT_ACC_WAIT_HINT 13 /* variant 3: suspend-time hint (ns) of the mbarrier waits; 0 = plain try_wait loop */
+#define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 = scheduling units visit the scene in a scattered order, 0 (default) = in order */
+#define SIM_OPT_ACC_INTERLEAVE 15 /* variant 3: scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
 #define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 

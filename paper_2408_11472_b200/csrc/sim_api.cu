@@ -82,6 +82,9 @@ struct sim_handle {
   int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
   int opt_ncw, opt_stages;          // warp-specialised kernel: compute warps per block, TMA ring depth (0 = auto)
   int ws_W, ws_stages, ws_blocks_per_sm;
+  int opt_wait_hint, opt_scatter, opt_ablate;
+  int opt_il;
+  int opt_pt, opt_epoch;            // v3: scatterers per lane per chunk; scatterers per fixed-point epoch (<= 2047)
   size_t smem_per_sm;
   // stats
   uint64_t launches, scatterers_seen;
@@ -205,7 +208,7 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
 
 int acc_blocks(const sim_handle* h) {
   if (h->opt_blocks > 0) return h->opt_blocks;
-  const int per_sm = h->opt_variant == 2 ? h->ws_blocks_per_sm : h->tile_blocks_per_sm;
+  const int per_sm = h->opt_variant >= 2 ? h->ws_blocks_per_sm : h->tile_blocks_per_sm;
   return h->sm_count * (per_sm > 0 ? per_sm : 1);
 }
 
@@ -218,26 +221,40 @@ cudaError_t plan_tile(sim_handle* h) {
   return e;
 }
 
+// Per-variant defaults of the warp-specialised kernels (measured on the 268M config, profiles/).
+void variant_defaults(sim_handle* h) {
+  if (h->opt_variant == 3) {
+    h->opt_ncw = 8; h->opt_pt = 4; h->opt_il = 2; h->opt_epoch = 8191;
+  } else {
+    h->opt_ncw = 14; h->opt_pt = 2; h->opt_il = 2; h->opt_epoch = 2047;
+  }
+}
+
 // Warp-specialised kernel: window width, ring depth and resident blocks per SM for the shared memory there is.
 cudaError_t plan_ws(sim_handle* h) {
-  const int G = h->cfg.n_gates, N = h->cfg.n_doppler, ncw = h->opt_ncw;
-  const int target = ncw <= 7 ? 4 : (ncw <= 14 ? 2 : 1);            // blocks per SM the register budget allows
+  const int G = h->cfg.n_gates, N = h->cfg.n_doppler, ncw = h->opt_ncw, pt = h->opt_pt;
+  const bool v3 = h->opt_variant == 3;
+  if (v3 && !acc_ws3_supported(ncw, pt, h->opt_il)) return cudaErrorInvalidValue;
+  if (!v3 && ncw != 7 && ncw != 14 && ncw != 22 && ncw != 30) return cudaErrorInvalidValue;
+  auto smem = [&](int g, int w, int st) { return v3 ? acc_ws3_smem_bytes(g, w, ncw, pt, st) : acc_ws_smem_bytes(g, w, ncw, st); };
+  const int target = v3 ? (ncw <= 4 ? 3 : ncw <= 14 ? 2 : 1) : ncw <= 7 ? 4 : (ncw <= 14 ? 2 : 1);   // blocks per SM the register budget allows
   size_t budget = h->smem_per_sm / target;
   budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
   if (budget > h->smem_optin - 1024) budget = h->smem_optin - 1024;
-  const size_t stage = acc_ws_smem_bytes(0, 0, ncw, 1);
+  const size_t stage = smem(0, 0, 1);
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
-  while (w > 1 && acc_ws_smem_bytes(G, w, ncw, 2) > budget) w >>= 1;
-  const size_t tiles = acc_ws_smem_bytes(G, w, ncw, 0);
+  while (w > 1 && smem(G, w, 2) > budget) w >>= 1;
+  const size_t tiles = smem(G, w, 0);
   int st = tiles + 2 * stage <= budget ? (int)((budget - tiles) / stage) : 2;
-  if (st > 4) st = 4;
+  const int st_max = v3 ? 6 : 4;
+  if (st > st_max) st = st_max;
   if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
   if (st < 2) st = 2;
   h->ws_W = w;
   h->ws_stages = st;
   int b = 1;
-  cudaError_t e = acc_ws_blocks_per_sm(G, w, ncw, st, &b);
+  cudaError_t e = v3 ? acc_ws3_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b) : acc_ws_blocks_per_sm(G, w, ncw, st, &b);
   h->ws_blocks_per_sm = b > 0 ? b : 1;
   return e;
 }
@@ -294,20 +311,41 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   const int blocks = acc_blocks(h);
   unsigned long long sc = (unsigned long long)h->opt_superchunk;
   if (sc == 0) {
-    // aim at >= 8 scheduling units per block, between one chunk and 64K scatterers
-    sc = 65536;
+    // aim at >= 8 scheduling units per block, between one chunk and 64K (v3: 16K) scatterers
+    sc = h->opt_variant == 3 ? 16384 : 65536;
     while (sc > (unsigned long long)kAccChunk && s->n / sc < (unsigned long long)blocks * 8) sc >>= 1;
   }
   unsigned long long unit = kAccChunk;
-  if (h->opt_variant == 2) {
-    const int ch = acc_ws_chunk(h->opt_ncw);
+  if (h->opt_variant >= 2) {
+    const int ch = h->opt_variant == 3 ? acc_ws3_chunk(h->opt_ncw, h->opt_pt) : acc_ws_chunk(h->opt_ncw);
     p.W = h->ws_W;
     p.stages = h->ws_stages;
-    p.epoch_chunks = 2047 / ch > 0 ? 2047 / ch : 1;
+    p.wait_hint = (unsigned)h->opt_wait_hint;
+    p.ablate = h->opt_ablate;
+    {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
+      const int L = (h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1) * ch;
+      int lg = 0;
+      while ((1 << lg) < L + 1) ++lg;
+      p.fx_cap = 31 - lg;
+      p.fx_target = p.fx_cap - 2 < 16 ? p.fx_cap - 2 : 16;
+    }
+    p.epoch_chunks = h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1;
     unit = (unsigned long long)ch * p.epoch_chunks;     // super-chunk = whole epochs: a jump never splits one
   }
   sc = (sc + unit - 1) / unit * unit;
   p.superchunk = sc;
+  {  // scattered visiting order: dark and illuminated parts of the scene are in flight at the same time, so the
+     // DRAM-bound and the compute-bound phases overlap instead of alternating
+    const unsigned long long n_sc = (s->n + sc - 1) / sc;
+    unsigned long long stride = 1;
+    if (h->opt_scatter && n_sc > 2) {
+      stride = (unsigned long long)((double)n_sc * 0.6180339887498949);
+      auto gcd = [](unsigned long long a, unsigned long long b) { while (b) { const unsigned long long t = a % b; a = b; b = t; } return a; };
+      while (stride > 1 && gcd(stride, n_sc) != 1) --stride;
+      if (stride < 1) stride = 1;
+    }
+    p.sc_stride = stride;
+  }
   p.index_path = h->opt_index_path;
   return p;
 }
@@ -316,7 +354,9 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
   AccParams p = make_acc_params(h, d_scat, sat, T);
   const int blocks = acc_blocks(h);
   int l = 0;
-  cudaError_t e = h->opt_variant == 2
+  cudaError_t e = h->opt_variant == 3
+                      ? launch_accumulate_ws3(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, h->stream, &l)
+                  : h->opt_variant == 2
                       ? launch_accumulate_ws(p, h->opt_ncw, blocks, h->stream, &l)
                       : launch_accumulate(p, h->opt_variant, h->opt_per_thread, h->opt_min_blocks, blocks, h->stream, &l);
   h->launches += l;
@@ -420,9 +460,12 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->stage_used[0] = h->stage_used[1] = false;
   h->n_updates = 0;
   h->pulses_emitted = 0;
-  h->opt_variant = 2;
-  h->opt_ncw = 14;
+  h->opt_variant = 3;
+  variant_defaults(h);
   h->opt_stages = 0;
+  h->opt_wait_hint = 0;
+  h->opt_scatter = 0;
+  h->opt_ablate = 0;
   h->opt_blocks = 0;
   h->opt_window = 0;
   h->opt_index_path = 1;
@@ -606,8 +649,12 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
   if (value < 0) return fail(h, SIM_ERR_INVALID_ARG, "option value < 0");
   switch (option) {
     case SIM_OPT_ACC_VARIANT:
-      if (value > 2) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
+      if (value > 3) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
       h->opt_variant = (int)value;
+      variant_defaults(h);   // warps, per-lane count and epoch length are per variant: back to that variant's defaults
+      if (value >= 2) {
+        if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      }
       return SIM_OK;
     case SIM_OPT_ACC_BLOCKS:
       if (value > 65535) return fail(h, SIM_ERR_INVALID_ARG, "too many blocks");
@@ -634,12 +681,54 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;
     case SIM_OPT_ACC_WARPS:
-      if (value != 7 && value != 14 && value != 22 && value != 30) return fail(h, SIM_ERR_INVALID_ARG, "compute warps per block: 7, 14, 22 or 30");
-      h->opt_ncw = (int)value;
-      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      {
+        const int old = h->opt_ncw;
+        h->opt_ncw = (int)value;
+        if (plan_ws(h) != cudaSuccess) {
+          h->opt_ncw = old;
+          plan_ws(h);
+          return fail(h, SIM_ERR_INVALID_ARG, "compute warps per block not supported by this accumulation variant");
+        }
+      }
+      return SIM_OK;
+    case SIM_OPT_ACC_PER_LANE:
+      {
+        const int old = h->opt_pt;
+        h->opt_pt = (int)value;
+        if (plan_ws(h) != cudaSuccess) {
+          h->opt_pt = old;
+          plan_ws(h);
+          return fail(h, SIM_ERR_INVALID_ARG, "scatterers per lane not supported by this accumulation variant");
+        }
+      }
+      return SIM_OK;
+    case SIM_OPT_ACC_WAIT_HINT:
+      h->opt_wait_hint = (int)value;
+      return SIM_OK;
+    case SIM_OPT_ACC_INTERLEAVE:
+      {
+        const int old = h->opt_il;
+        h->opt_il = (int)value;
+        if (plan_ws(h) != cudaSuccess) {
+          h->opt_il = old;
+          plan_ws(h);
+          return fail(h, SIM_ERR_INVALID_ARG, "interleave not supported by this accumulation variant");
+        }
+      }
+      return SIM_OK;
+    case SIM_OPT_ACC_SCATTER:
+      h->opt_scatter = value != 0;
+      return SIM_OK;
+    case 99:
+      h->opt_ablate = (int)value;
+      return SIM_OK;
+    case SIM_OPT_ACC_EPOCH:
+      if (value < 64 || value > 65535 || (h->opt_variant != 3 && value > 2047))
+        return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..2047 (variant 3: ..65535)");
+      h->opt_epoch = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_STAGES:
-      if (value > 4 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..4");
+      if (value > 6 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..6 (variant 2: at most 4)");
       h->opt_stages = (int)value;
       if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       return SIM_OK;

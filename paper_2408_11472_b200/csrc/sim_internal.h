@@ -65,6 +65,10 @@ struct AccParams {
   float a0, a1, a2;       // 1/R^2 = a0 + gfx (a1 + gfx a2), gfx = gf * 2^kFracBits
   float w_scale;          // 2^-kFracBits
   int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
+  int fx_cap, fx_target;     // v3 block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
+  unsigned long long sc_stride;  // v3: super-chunk visited by ticket t is (t * sc_stride) mod n_superchunks (coprime)
+  int ablate;                // debug: 1 = skip the shared-memory adds, 2 = skip the amplitude (timing experiments only)
+  unsigned wait_hint;        // v3: suspend-time hint of the mbarrier waits in ns (0 = plain try_wait loop)
 };
 
 struct SynParams {
@@ -89,6 +93,12 @@ size_t acc_ws_smem_bytes(int G, int W, int ncw, int stages);
 cudaError_t acc_ws_blocks_per_sm(int G, int W, int ncw, int stages, int* blocks);
 cudaError_t launch_accumulate_ws(const AccParams& p, int ncw, int blocks, cudaStream_t st, int* launches);
 int acc_ws_chunk(int ncw);
+// v3: producer warp + drain warp + ncw compute warps, pt scatterers per lane per chunk
+size_t acc_ws3_smem_bytes(int G, int W, int ncw, int pt, int stages);
+bool acc_ws3_supported(int ncw, int pt, int il);
+cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
+cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, int blocks, cudaStream_t st, int* launches);
+int acc_ws3_chunk(int ncw, int pt);
 cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
                            int* launches);
 size_t acc_tile_smem_bytes(int G, int W, int per_thread);

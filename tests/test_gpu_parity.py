@@ -32,7 +32,7 @@ def _indices_exact(orc, sim_mod, wl, scat_cuda, scat_np, sim, u=0, index_path=No
 
 
 # ---- configs[0]: Tiny, full size, every accumulation variant ----------------------------------------
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_tiny_full(oracle, sim_mod, variant):
     wl = W.get("tiny")
     scat = W.scatterers(wl)
@@ -65,7 +65,7 @@ def test_reduced_configs(oracle, sim_mod, name):
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
     assert np.abs(T_ref).max() > 0
-    for variant in (0, 1, 2):
+    for variant in (0, 1, 2, 3):
         T, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda, options={sim_mod.OPT_ACC_VARIANT: variant})
         U.check_stream(oracle, wl, T, iq, T_ref)
     for u in (0, wl.n_updates - 1):
@@ -187,7 +187,7 @@ def test_append_equals_single_call_and_linearity(oracle, sim_mod):
 
 # ---- edge cases ------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n", [0, 1, 3, 4, 5, 2047, 2048, 2049, 3 * 2048 + 5])
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_ragged_sizes(oracle, sim_mod, n, variant):
     wl = W.get("tiny").scaled(n_updates=1)
     scat = {k: v[:n].contiguous() for k, v in W.scatterers(wl).items()}
@@ -202,7 +202,7 @@ def test_ragged_sizes(oracle, sim_mod, n, variant):
         _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_degenerate_inputs(oracle, sim_mod, variant):
     """Out-of-window, dead (s0dA <= 0, NaN), non-finite positions/velocities: dropped on both sides."""
     wl = W.get("tiny").scaled(n_updates=1)
@@ -328,6 +328,55 @@ def test_heavy_tailed_amplitudes(oracle, sim_mod):
     T_ref = U.oracle_spectra(oracle, wl, dim_np, [0])[0]
     sim.accumulate_update(dim, sim_mod.sat_for(wl, 0))
     assert U.rel_l2(sim.get_spectrum(1).cpu().numpy(), T_ref) <= U.TOL
+
+
+V3_SHAPES = [(8, 2, 2), (8, 4, 4), (8, 4, 2), (12, 2, 2), (12, 4, 2), (16, 4, 2), (20, 4, 2), (28, 2, 2)]
+
+
+@pytest.mark.parametrize("ncw,pt,il", V3_SHAPES)
+def test_v3_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
+    """Production kernel (variant 3): every compiled block shape, short to very long fixed-point epochs (the
+    admitted magnitude range shrinks as the epoch grows so that no cell can overflow), scattered visiting
+    order, tiny scheduling units, on a scene with out-of-window parts and a ragged tail."""
+    wl = W.get("sar_footprint_268m").scaled(n_along=509, n_cross=1031, spacing_m=13.0, n_updates=1)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 1}), (4095, {sim_mod.OPT_ACC_STAGES: 2}),
+                         (8191, {sim_mod.OPT_ACC_SUPERCHUNK: 1}), (16383, {}), (65535, {sim_mod.OPT_ACC_BLOCKS: 3})):
+        sim = sim_mod.Sim(sim_mod.config_for(wl))
+        sim.set_option(sim_mod.OPT_ACC_VARIANT, 3)
+        sim.set_option(sim_mod.OPT_ACC_PER_LANE, pt)        # each intermediate combination is a compiled shape
+        sim.set_option(sim_mod.OPT_ACC_WARPS, ncw)
+        sim.set_option(sim_mod.OPT_ACC_INTERLEAVE, il)
+        sim.set_option(sim_mod.OPT_ACC_EPOCH, epoch)
+        for k, v in extra.items():
+            sim.set_option(k, v)
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+        e = U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref)
+        assert e <= U.TOL, (ncw, pt, il, epoch, e)
+
+
+def test_coherent_pileup_cannot_overflow(oracle, sim_mod):
+    """Worst case for the int32 tiles: every scatterer of a long epoch lands in the SAME cell with the SAME
+    phase (identical positions and velocities), amplitudes up to just below the admitted maximum."""
+    wl = W.get("tiny").scaled(n_updates=1)
+    n = 300_000
+    g = torch.Generator().manual_seed(7)
+    ratio = torch.tensor([1.0, 1.9, 3.9, 0.3])[torch.randint(0, 4, (n,), generator=g)]
+    scat = {"x": torch.zeros(n), "y": torch.zeros(n), "z": torch.full((n,), 0.1), "vx": torch.zeros(n),
+            "vy": torch.zeros(n), "vz": torch.zeros(n), "s0dA": 10.0 * ratio * ratio}
+    scat = {k: v.float().contiguous() for k, v in scat.items()}
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    assert (np.abs(T_ref) > 0).sum() == 2                       # one bin, two gate halves
+    for variant, epoch in ((2, 2047), (3, 2047), (3, 8191), (3, 16383), (3, 65535)):
+        sim = sim_mod.Sim(sim_mod.config_for(wl))
+        sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
+        sim.set_option(sim_mod.OPT_ACC_EPOCH, epoch)
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+        e = U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref)
+        assert e <= U.TOL, (variant, epoch, e)
 
 
 def test_maximum_sizes(oracle, sim_mod):
