@@ -167,7 +167,7 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_WARPS 9      /* variant 2: compute warps per block: 7, 14 (default), 22 or 30 */
 #define SIM_OPT_ACC_STAGES 10    /* variant 2: depth of the TMA stage ring, 2..4; 0 = as many as fit */
 #define SIM_OPT_ACC_PER_LANE 11  /* variant 3: scatterers per lane per chunk: 2 or 4 */
-#define SIM_OPT_ACC_EPOCH 12     /* variants 2, 3: scatterers per fixed-point epoch, 64..2047 (default 2047) */
+#define SIM_OPT_ACC_EPOCH 12     /* scatterers per fixed-point epoch: variant 2 64..2047 (default 2047), variant 3 64..16383 (default 8191) */
 #define SIM_OPT_ACC_WAIT_HINT 13 /* variant 3: suspend-time hint (ns) of the mbarrier waits; 0 = plain try_wait loop */
 #define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 = scheduling units visit the scene in a scattered order, 0 (default) = in order */
 #define SIM_OPT_ACC_INTERLEAVE 15 /* variant 3: scatterers in flight per lane at a time: 2 or 4 (<= per lane) */

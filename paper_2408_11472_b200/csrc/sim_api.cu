@@ -723,8 +723,8 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       h->opt_ablate = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_EPOCH:
-      if (value < 64 || value > 65535 || (h->opt_variant != 3 && value > 2047))
-        return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..2047 (variant 3: ..65535)");
+      if (value < 64 || value > 16383 || (h->opt_variant != 3 && value > 2047))
+        return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..2047 (variant 3: ..16383)");
       h->opt_epoch = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_STAGES:
