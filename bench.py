@@ -24,6 +24,7 @@ if ROOT not in sys.path:
 
 import torch  # noqa: E402
 
+from paper_2408_11472_b200 import dist as D  # noqa: E402
 from paper_2408_11472_b200 import workloads as W  # noqa: E402
 
 DEFAULT_WORKLOAD = "sar_footprint_268m"   # configs[2]: the config north_star quotes the roofline target on
@@ -106,17 +107,6 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------------------
-def shard(scat, rank, world, n_cross):
-    """Rows (along-track lines) [lo, hi) of the scene for this rank: the path shards over scatterers
-    (the spectrum is a sum over scatterers); one all-reduce per update joins them."""
-    if world == 1:
-        return scat
-    n = scat["x"].numel()
-    rows = n // n_cross
-    lo, hi = rows * rank // world * n_cross, rows * (rank + 1) // world * n_cross
-    return {k: v[lo:hi].contiguous() for k, v in scat.items()}
-
-
 def cpu_oracle_sample(wl, scat_cpu, nthreads, target_s=12.0):
     """Times the oracle, as it stands, on a bounded sample of the workload: passes of one update over the
     central block of ns scatterers (satellite states of successive updates) until about target_s seconds of
@@ -227,7 +217,7 @@ def main():
 
     U, P, G, N = wl.n_updates, wl.pulses_per_update, wl.n_gates, wl.n_doppler
     scat_full = W.scatterers(wl, device=dev)
-    scat = shard(scat_full, rank, world, wl.n_cross)
+    scat = D.shard_scatterers(scat_full, wl.n_cross, rank, world)
     if world > 1:
         del scat_full
     n_local = scat["x"].numel()
@@ -253,7 +243,7 @@ def main():
                 e1.record(stream)
                 acc_events.append((e0, e1))
             if world > 1:   # the one exchange step: partial spectra -> full spectrum
-                dist.all_reduce(sim.spectrum_view(sim.stats()["updates_accumulated"] - 1))
+                D.allreduce_spectrum(sim.spectrum_view(sim.stats()["updates_accumulated"] - 1))
         sim.synthesize_pulses(U * P, iq, flags=S.SYN_FINAL)
 
     def barrier():
@@ -305,7 +295,7 @@ def main():
             for u in range(U):
                 sim_h.accumulate_update_host(host, sats[u])
                 if world > 1:
-                    dist.all_reduce(sim_h.spectrum_view(sim_h.stats()["updates_accumulated"] - 1))
+                    D.allreduce_spectrum(sim_h.spectrum_view(sim_h.stats()["updates_accumulated"] - 1))
             sim_h.synthesize_pulses_host(U * P, iq_h, flags=S.SYN_FINAL)
 
         step_h()
