@@ -419,7 +419,7 @@ int do_synthesize(sim_handle* h, int64_t n_pulses, float2* d_iq, int64_t s_first
   p.logN = 0;
   while ((1 << p.logN) < p.N) ++p.logN;
   p.P = h->cfg.pulses_per_update;
-  p.GT = synth_gate_tile(p.N);
+  p.GT = synth_gate_tile(p.N, p.G, s_last - s_first + 1, h->sm_count);
   p.weight_mode = h->cfg.weight_mode;
   int l = 0;
   cudaError_t e = launch_synthesize(p, (int)(s_last - s_first + 1), h->stream, &l);
@@ -498,6 +498,12 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   e = plan_tile(h);
   if (e == cudaSuccess) e = plan_ws(h);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
+  {
+    int logN = 0;
+    while ((1 << logN) < cfg->n_doppler) ++logN;
+    e = synth_prepare(logN);
+    if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "synthesis kernel shared-memory attribute"); }
+  }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters)"); }
   int l = 0;

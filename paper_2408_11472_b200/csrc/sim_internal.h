@@ -105,6 +105,7 @@ size_t acc_tile_smem_bytes(int G, int W, int per_thread);
 cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
-int synth_gate_tile(int N);
+int synth_gate_tile(int N, int G, long long n_segments, int sm_count);
+cudaError_t synth_prepare(int logN);
 
 }  // namespace simk
