@@ -6,10 +6,10 @@
 // after the v2 profile (profiles/r01_v2_ws_kernel.md):
 //   * three roles instead of two: warps 0..NCW-1 compute (NCW a multiple of 4: the same number on every SM
 //     sub-partition), warp NCW only PRODUCES (ticket counter -> TMA bulk copies, next ticket prefetched), warp
-//     NCW+1 only DRAINS finished tiles (step A7); both poll politely (nanosleep).  A drain no longer delays
+//     NCW+1 only DRAINS finished tiles (step A7); both sleep in hardware-suspended mbarrier waits.  A drain no longer delays
 //     the next loads;
-//   * every wait is a hardware-suspended mbarrier.try_wait with a time hint: v2 spent 20 % of its issue slots
-//     spinning;
+//   * the two control warps wait with a suspend-time hint (v2 spent 20 % of its issue slots spinning); the block's
+//     end is signalled through the barriers themselves (the compute warps publish the index of the final epoch);
 //   * the tile has one padding row below gate 0 and one above gate G-1, so the two gate halves need no
 //     per-half bounds predicate;
 //   * fewer compute warps with more registers each (no spills), loop state kept in registers.
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
   __shared__ __align__(8) unsigned long long s_full[kW3MaxStages], s_empty[kW3MaxStages], s_tdone[2], s_tfree[2];
   __shared__ __align__(16) unsigned s_desc[kW3MaxStages][4];
   __shared__ int s_slot[4][kS3Ints];
-  __shared__ unsigned s_nepochs;
+  __shared__ unsigned s_last;   // index of the block's final epoch, written by the compute warps when they see the end marker
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int S = p.stages, EC = p.epoch_chunks;
@@ -121,7 +121,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
   const unsigned full0 = sh::addr(&s_full[0]), empty0 = sh::addr(&s_empty[0]);
   const unsigned tdone0 = sh::addr(&s_tdone[0]), tfree0 = sh::addr(&s_tfree[0]);
   const unsigned desc0 = sh::addr(&s_desc[0][0]), slot0 = sh::addr(&s_slot[0][0]);
-  const unsigned nep_a = sh::addr(&s_nepochs);
+  const unsigned last_a = sh::addr(&s_last);
 
   for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * (NCW + 2) * 32) sh::st(tile0 + a, 0);
   if (tid < 4) {
@@ -130,7 +130,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
     sh::st(slot0 + 4u * kS3Ints * tid + 4 * kS3Gmax, INT_MIN);
   }
   if (tid == 0) {
-    sh::st(nep_a, (int)kFull);
+    sh::st(last_a, (int)kFull);
     for (int s = 0; s < S; ++s) {
       sh::mbar_init(full0 + 8u * s, 1);
       sh::mbar_init(empty0 + 8u * s, NCW);
@@ -150,27 +150,20 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
     Cursor3 cur{0, 0, atomicAdd(&p.counters[kCtrTicket], 1u), false};
     unsigned stg = 0, ph = 0;
     for (unsigned c = 0;; ++c) {
-      if (c >= (unsigned)S) {   // chunk c - S pulled out of the stage (polite poll: this lane shares an SMSP with compute warps)
-        while (!sh::mbar_try_wait(empty0 + 8u * stg, ph ^ 1u, 1000u)) __nanosleep(p.wait_hint ? p.wait_hint : 40u);
-      }
+      // chunk c - S pulled out of the stage.  Suspended wait: this lane shares an SM sub-partition with compute warps
+      if (c >= (unsigned)S) sh::mbar_wait_sleepy(empty0 + 8u * stg, ph ^ 1u, 100000u);
       const unsigned nv = produce_chunk3<CH>(p, cur, n_sc, stage0 + stg * kStageBytes, desc0 + 16u * stg, full0 + 8u * stg);
-      if (nv == 0) {   // the end marker is out: c real chunks, ceil(c / EC) epochs
-        sh::st_release(nep_a, (int)((c + (unsigned)EC - 1u) / (unsigned)EC));
-        return;
-      }
+      if (nv == 0) return;   // the end marker is out
       if (++stg == (unsigned)S) { stg = 0; ph ^= 1u; }
     }
   }
 
   if (warp == NCW + 1) {
     // ================= drain warp: tile of epoch e -> T (step A7), tile handed back =================
-    const int logW = 31 - __clz(W);
+    const int logW = W > 1 ? 32 - __clz(W - 1) : 0, Wp = 1 << logW;   // window rounded up to a power of two: lanes kw >= W idle
     for (unsigned e = 0;; ++e) {
       const unsigned b = e & 1u;
-      while (!sh::mbar_try_wait(tdone0 + 8u * b, (e >> 1) & 1u, 20000u)) {   // every compute warp finished epoch e
-        if ((unsigned)sh::ld_acquire(nep_a) <= e) return;                    // ... or there is no epoch e
-        __nanosleep(200u);
-      }
+      sh::mbar_wait_sleepy(tdone0 + 8u * b, (e >> 1) & 1u, 100000u);   // every compute warp finished epoch e
       const unsigned slot = slot0 + 4u * kS3Ints * (e & 3u);
       if (sh::ld(slot + 4 * kS3State) == kT3Ready) {
         const int k0 = sh::ld(slot + 4 * kS3K0), ex = sh::ld(slot + 4 * kS3Ex);
@@ -179,7 +172,8 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
         const int ncell = (r1 >= r0) ? (r1 - r0 + 1) << logW : 0;   // nothing fitted (all escaped): empty range
         const unsigned tile = tile0 + b * tile_bytes;
         for (int cc = lane; cc < ncell; cc += 32) {
-          const int r = r0 + (cc >> logW), kw = cc & (W - 1);
+          const int r = r0 + (cc >> logW), kw = cc & (Wp - 1);
+          if (kw >= W) continue;
           const unsigned a = tile + 4u * (unsigned)((r + 1) * RS + kw);
           const int re = sh::ld(a), im = sh::ld(a + plane_bytes);
           if (re | im) {
@@ -197,6 +191,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
       }
       __syncwarp();
       if (lane == 0) sh::mbar_arrive(tfree0 + 8u * b);  // release: zeroed tile and reset slot are visible
+      if ((unsigned)sh::ld(last_a) == e) return;        // written before the last arrival on tdone of epoch e
     }
   }
 
@@ -274,8 +269,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
         for (int j = 0; j < IL; ++j) {
           ok[j] = index_part<FAST>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], fallbacks);
           float A;
-          if (p.ablate & 2) { A = 4e-12f; c[j] = make_float2(A * ix[j].fr, A * ix[j].w1); }
-          else c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
+          c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
           ab[j] = __float_as_int(A);
           any |= ok[j];
         }
@@ -337,7 +331,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
           const bool fits = ok[j] && kw < (unsigned)W && (unsigned)(ab[j] - lo_bits) <= fx_span;
           const float w1s = ix[j].w1 * s, w0s = s - w1s;
           const unsigned a0 = tile_b + 4u * (unsigned)((ix[j].g0 + 1) * RS + (int)kw);   // row g0 (padded by one)
-          if (fits && !(p.ablate & 1)) {
+          if (fits) {
             sh::red_add(a0, fx_round3(c[j].x, w0s));
             sh::red_add(a0 + plane_bytes, fx_round3(c[j].y, w0s));
             sh::red_add(a0 + 4u * (unsigned)RS, fx_round3(c[j].x, w1s));
@@ -364,7 +358,8 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
     }
 
     // ---- end of an epoch (or of the input inside one): row range of what this warp added, tile to the drain warp ----
-    if (ci != 0 || more) {
+    {
+      if (!more && lane == 0) sh::st(last_a, (int)e);   // the final epoch (possibly empty): the drain warp stops after it
       if (have) {
         gmin = __reduce_min_sync(kFull, gmin);
         gmax = __reduce_max_sync(kFull, gmax);
@@ -389,8 +384,7 @@ typedef void (*W3Kernel)(AccParams);
 static W3Kernel ws3_kernel(int ncw, int pt, int il, bool fast) {
 #define W3_CASE(NCW_, PT_, IL_) \
   if (ncw == NCW_ && pt == PT_ && il == IL_) return fast ? acc_ws3_kernel<NCW_, PT_, IL_, true> : acc_ws3_kernel<NCW_, PT_, IL_, false>;
-  W3_CASE(8, 2, 2) W3_CASE(8, 4, 4) W3_CASE(8, 4, 2) W3_CASE(12, 2, 2) W3_CASE(12, 4, 2) W3_CASE(14, 2, 2)
-  W3_CASE(16, 2, 2) W3_CASE(16, 4, 4) W3_CASE(16, 4, 2) W3_CASE(20, 2, 2) W3_CASE(20, 4, 2) W3_CASE(20, 4, 4) W3_CASE(24, 2, 2) W3_CASE(28, 2, 2)
+  W3_CASE(8, 2, 2) W3_CASE(8, 4, 4) W3_CASE(8, 4, 2) W3_CASE(12, 2, 2) W3_CASE(16, 4, 2) W3_CASE(20, 4, 2)
 #undef W3_CASE
   return nullptr;
 }

@@ -82,7 +82,7 @@ struct sim_handle {
   int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
   int opt_ncw, opt_stages;          // warp-specialised kernel: compute warps per block, TMA ring depth (0 = auto)
   int ws_W, ws_stages, ws_blocks_per_sm;
-  int opt_wait_hint, opt_scatter, opt_ablate;
+  int opt_wait_hint, opt_scatter;
   int opt_il;
   int opt_pt, opt_epoch;            // v3: scatterers per lane per chunk; scatterers per fixed-point epoch (<= 2047)
   size_t smem_per_sm;
@@ -138,6 +138,7 @@ int choose_window(const sim_handle* h) {
   const int G = h->cfg.n_gates, N = h->cfg.n_doppler;
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
+  while (w & (w - 1)) w &= w - 1;   // this kernel needs a power of two
   // default: at most 32 KB of tile next to the stages; an explicit window may use all of shared memory
   const size_t stages = acc_tile_smem_bytes(0, 0, h->opt_per_thread);
   const size_t budget = h->opt_window > 0 ? (h->smem_optin > 8192 ? h->smem_optin - 4096 : 4096) : stages + 32 * 1024;
@@ -244,9 +245,22 @@ cudaError_t plan_ws(sim_handle* h) {
   const size_t stage = smem(0, 0, 1);
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
-  while (w > 1 && smem(G, w, 2) > budget) w >>= 1;
-  const size_t tiles = smem(G, w, 0);
+  if (!v3) while (w & (w - 1)) w &= w - 1;   // variant 2 needs a power of two
+  while (w > 1 && smem(G, w, 2) > budget) w = v3 ? w - 1 : w >> 1;   // v3 takes any width
+  size_t tiles = smem(G, w, 0);
   int st = tiles + 2 * stage <= budget ? (int)((budget - tiles) / stage) : 2;
+  if (v3 && h->opt_window == 0 && st < 3) {
+    // a third stage is worth more than the last bins of the window (measured: 16 bins x 2 stages 1.42 ms,
+    // 12 bins x 3 stages 1.39 ms on the 268M config; below 12 bins the escapes take over)
+    for (int w2 = w - 1; w2 >= 12 && w2 >= 3 * w / 4; --w2) {
+      if (smem(G, w2, 0) + 3 * stage <= budget) {
+        w = w2;
+        tiles = smem(G, w, 0);
+        st = 3;
+        break;
+      }
+    }
+  }
   const int st_max = v3 ? 6 : 4;
   if (st > st_max) st = st_max;
   if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
@@ -321,7 +335,6 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
     p.W = h->ws_W;
     p.stages = h->ws_stages;
     p.wait_hint = (unsigned)h->opt_wait_hint;
-    p.ablate = h->opt_ablate;
     {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
       const int L = (h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1) * ch;
       int lg = 0;
@@ -465,7 +478,6 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->opt_stages = 0;
   h->opt_wait_hint = 0;
   h->opt_scatter = 0;
-  h->opt_ablate = 0;
   h->opt_blocks = 0;
   h->opt_window = 0;
   h->opt_index_path = 1;
@@ -670,7 +682,7 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       h->opt_superchunk = value;
       return SIM_OK;
     case SIM_OPT_ACC_WINDOW_BINS:
-      if (value & (value - 1)) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two");
+      if (h->opt_variant != 3 && (value & (value - 1))) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two (any width with variant 3)");
       if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
       h->opt_window = (int)value;
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
@@ -724,9 +736,6 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       return SIM_OK;
     case SIM_OPT_ACC_SCATTER:
       h->opt_scatter = value != 0;
-      return SIM_OK;
-    case 99:
-      h->opt_ablate = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_EPOCH:
       if (value < 64 || value > 16383 || (h->opt_variant != 3 && value > 2047))

@@ -67,7 +67,6 @@ struct AccParams {
   int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
   int fx_cap, fx_target;     // v3 block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
   unsigned long long sc_stride;  // v3: super-chunk visited by ticket t is (t * sc_stride) mod n_superchunks (coprime)
-  int ablate;                // debug: 1 = skip the shared-memory adds, 2 = skip the amplitude (timing experiments only)
   unsigned wait_hint;        // v3: suspend-time hint of the mbarrier waits in ns (0 = plain try_wait loop)
 };
 
