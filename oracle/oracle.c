@@ -22,7 +22,9 @@
  *                            (PAPER.md:100-101); eq. (1) at PAPER.md:61, W_i(x) = (1 - |i-x|/n_fast)^(1/2).
  *
  * Pins: every function here is pinned by tests/test_oracle_pins.py (closed forms, numpy.fft
- * special case, Parseval, brute-force regular-mode sum, an independent numpy restatement).
+ * special case, Parseval, brute-force regular-mode sum, an independent numpy restatement); the
+ * pulse-pair Doppler mode by tests/test_oracle_pulse_pair.py (the literal arg(C_{i+1} C_i^*) estimator at
+ * 50 digits, the analytic f_D plus its closed-form second-order term, aliasing).
  * Parity unpinned BY THE PAPER (fixed only by DESIGN.md readings): the analytic antenna gain
  * G(theta) (A10), the tail rule for a missing successor spectrum (A3), the nearest-bin rule (A7).
  *
@@ -40,6 +42,9 @@
 #define ORACLE_W_SQRT 0   /* paper eq. (1) */
 #define ORACLE_W_LINEAR 1 /* partition of unity (north_star wording), reading A1 */
 
+#define ORACLE_DOPPLER_ANALYTIC 0   /* f_D = -2 (v_p - v_sat).u / lambda (north_star; reading A5) */
+#define ORACLE_DOPPLER_PULSE_PAIR 1 /* the paper's estimator, Algorithm 1 lines 5-7 (readings A6, R4) */
+
 #define ORACLE_GATE_NONE INT32_MIN /* scatterer touches no gate of the window / is dropped */
 
 typedef struct {
@@ -51,6 +56,7 @@ typedef struct {
   double prf_hz;             /* PRF */
   double gate_spacing_m;     /* Delta R */
   double antenna_alpha;      /* G(theta) = exp(-alpha sin^2 theta), reading A10 */
+  int32_t doppler_mode;      /* ORACLE_DOPPLER_* */
 } oracle_config;
 
 typedef struct {
@@ -69,7 +75,7 @@ static const double TWO_PI = 6.283185307179586476925286766559;
 typedef struct {
   int32_t g0, k;
   double w0, w1; /* two-gate linear weights, reading A8 */
-  double R, R2, fr;
+  double R, R2, fr, kf;
   double dx, dy, dz;
 } geom_t;
 
@@ -88,15 +94,32 @@ static int geometry(const oracle_config *c, const oracle_sat *s, double inv_dR,
   const double dvx = (double)vxf - s->vel[0];
   const double dvy = (double)vyf - s->vel[1];
   const double dvz = (double)vzf - s->vel[2];
-  /* rdot = dR/dt = (v_p - v_sat).u,  u = (r_p - r_sat)/R ;  f_D = -2 rdot / lambda (reading A5) */
-  const double rdot = fma(dvz, dz, fma(dvy, dy, dvx * dx)) / R;
-  const double kf = rdot * cD; /* = f_D * N / PRF */
+  double kf;
+  if (c->doppler_mode == ORACLE_DOPPLER_PULSE_PAIR) {
+    /* Algorithm 1 lines 5-7: update_simulation((i n_fast + 1)/PRF), C_{i+1}, then
+     * D_i = arg(C_{i+1} C_i^*) PRF / (2 pi)  (physical form of the printed formula, reading A6).
+     * Scatterer and satellite both move at constant velocity over one PRI = 1/PRF, so the offset one
+     * pulse later is d' = d + (v_p - v_sat)/PRF and, with C ~ exp(-i 4 pi R / lambda),
+     * arg(C_{i+1} C_i^*) = -4 pi (R' - R)/lambda (mod 2 pi):  f_D N/PRF = -(2N/lambda)(R' - R) (mod N).
+     * The wrap of arg() is the "mod N" of the bin (natural aliasing).  Basic IEEE operations only, so
+     * that the GPU can reproduce the bin bit for bit (reading R4). */
+    const double pri = 1.0 / c->prf_hz;
+    const double cP = (-2.0 * (double)c->n_doppler) / c->wavelength_m;
+    const double dx1 = fma(dvx, pri, dx), dy1 = fma(dvy, pri, dy), dz1 = fma(dvz, pri, dz);
+    const double R1 = sqrt(fma(dz1, dz1, fma(dy1, dy1, dx1 * dx1)));
+    kf = (R1 - R) * cP;
+  } else {
+    /* rdot = dR/dt = (v_p - v_sat).u,  u = (r_p - r_sat)/R ;  f_D = -2 rdot / lambda (reading A5) */
+    const double rdot = fma(dvz, dz, fma(dvy, dy, dvx * dx)) / R;
+    kf = rdot * cD; /* = f_D * N / PRF */
+  }
   if (!(fabs(kf) < 1073741824.0)) return 0; /* |kf| >= 2^30 or NaN: dropped */
   const double kk = floor(kf + 0.5); /* nearest bin, ties up (reading A7) */
   const double N = (double)c->n_doppler;
   const double kmod = kk - N * floor(kk / N); /* in [0,N): negative Doppler wraps to k+N (A2) */
   const double q = R * two_over_lambda;       /* 2R/lambda, in cycles */
   o->g0 = (int32_t)g0d;
+  o->kf = kf;
   o->k = (int32_t)kmod;
   o->w1 = gf - g0d;
   o->w0 = 1.0 - o->w1;
@@ -211,6 +234,22 @@ int oracle_indices(const oracle_config *c, const oracle_sat *s, int64_t n, const
       g0[p] = ORACLE_GATE_NONE;
       k[p] = -1;
     }
+  }
+  return 0;
+}
+
+/* Doppler coordinate kf = f_D N / PRF before rounding to a bin (pins of the Doppler readings); NaN for
+ * a dropped scatterer. */
+int oracle_doppler_coordinate(const oracle_config *c, const oracle_sat *s, int64_t n, const float *x,
+                              const float *y, const float *z, const float *vx, const float *vy,
+                              const float *vz, double *kf) {
+  if (!c || !s || n < 0) return -1;
+  double inv_dR, two_over_lambda, cD;
+  constants(c, &inv_dR, &two_over_lambda, &cD);
+  for (int64_t p = 0; p < n; ++p) {
+    geom_t g;
+    kf[p] = geometry(c, s, inv_dR, two_over_lambda, cD, x[p], y[p], z[p], vx[p], vy[p], vz[p], &g)
+                ? g.kf : NAN;
   }
   return 0;
 }

@@ -18,6 +18,8 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 
 W_SQRT = 0
 W_LINEAR = 1
+DOPPLER_ANALYTIC = 0
+DOPPLER_PULSE_PAIR = 1
 GATE_NONE = -(2**31)
 
 
@@ -31,6 +33,7 @@ class OracleConfig(C.Structure):
         ("prf_hz", C.c_double),
         ("gate_spacing_m", C.c_double),
         ("antenna_alpha", C.c_double),
+        ("doppler_mode", C.c_int32),
     ]
 
 
@@ -69,6 +72,9 @@ def lib():
         L.oracle_indices.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
                                      fp, fp, fp, fp, fp, fp, ip, ip]
         L.oracle_indices.restype = C.c_int
+        L.oracle_doppler_coordinate.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
+                                                fp, fp, fp, fp, fp, fp, dp]
+        L.oracle_doppler_coordinate.restype = C.c_int
         L.oracle_idft.argtypes = [C.c_int32, C.c_int32, dp, dp]
         L.oracle_idft.restype = C.c_int
         L.oracle_weight.argtypes = [C.c_int32, C.c_int32, C.c_int64]
@@ -82,10 +88,10 @@ def lib():
 
 
 def make_config(n_gates, n_doppler, pulses_per_update, wavelength_m, prf_hz, gate_spacing_m,
-                antenna_alpha, weight_mode=W_SQRT) -> OracleConfig:
+                antenna_alpha, weight_mode=W_SQRT, doppler_mode=DOPPLER_ANALYTIC) -> OracleConfig:
     return OracleConfig(int(n_gates), int(n_doppler), int(pulses_per_update), int(weight_mode),
                         float(wavelength_m), float(prf_hz), float(gate_spacing_m),
-                        float(antenna_alpha))
+                        float(antenna_alpha), int(doppler_mode))
 
 
 def make_sat(pos, vel, boresight, range_gate0_m) -> OracleSat:
@@ -136,6 +142,18 @@ def indices(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz):
     if rc < 0:
         raise RuntimeError(f"oracle_indices failed: {rc}")
     return g0, k
+
+
+def doppler_coordinate(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz):
+    """kf = f_D N / PRF per scatterer before rounding to a bin (NaN when dropped)."""
+    arrs = [_f32(a) for a in (x, y, z, vx, vy, vz)]
+    n = arrs[0][0].size
+    kf = np.empty(n, dtype=np.float64)
+    rc = lib().oracle_doppler_coordinate(C.byref(cfg), C.byref(sat), n, *[a[1] for a in arrs],
+                                         kf.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc < 0:
+        raise RuntimeError(f"oracle_doppler_coordinate failed: {rc}")
+    return kf
 
 
 def idft(T):
