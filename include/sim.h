@@ -44,6 +44,14 @@ extern "C" {
 #define SIM_ACC_APPEND 1u /* sim_accumulate_update: add to the current update instead of starting one */
 #define SIM_SYN_FINAL 1u  /* sim_synthesize_pulses: a missing successor spectrum is allowed (tail rule) */
 
+/* Doppler source of step A4.
+ *   SIM_DOPPLER_ANALYTIC:   f_D = -2 (v_p - v_sat).u / lambda  (north_star; reading A5).
+ *   SIM_DOPPLER_PULSE_PAIR: the paper's estimator, Algorithm 1 lines 5-7: the scene one
+ *     PRI later (scatterers and satellite moved by v / PRF), D = arg(C_{i+1} C_i^*) PRF / 2 pi
+ *     = -2 (R' - R) PRF / lambda, aliased into the N bins (readings A6, R4). */
+#define SIM_DOPPLER_ANALYTIC 0
+#define SIM_DOPPLER_PULSE_PAIR 1
+
 #define SIM_GATE_NONE INT32_MIN /* sim_debug_indices: scatterer touches no gate / is dropped */
 
 typedef struct sim_handle sim_handle; /* opaque, host memory, owned by the library */
@@ -56,6 +64,7 @@ typedef struct sim_config {
   int32_t max_pending_updates; /* spectra kept in the ring, >= 2 */
   int32_t weight_mode;         /* SIM_W_SQRT (default, the paper) or SIM_W_LINEAR */
   int32_t device;              /* CUDA device ordinal the workspace and stream live on */
+  int32_t doppler_mode;        /* SIM_DOPPLER_ANALYTIC (default) or SIM_DOPPLER_PULSE_PAIR */
   double wavelength_m;         /* lambda > 0 */
   double prf_hz;               /* PRF > 0 */
   double gate_spacing_m;       /* Delta R > 0 */

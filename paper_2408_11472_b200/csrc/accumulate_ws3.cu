@@ -377,6 +377,35 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Index-only kernel (parity pin P11, sim_debug_indices): the index routine of the production kernel
+// (pre_part + index_part of scatter_math.cuh), one scatterer per thread, s0dA not consulted.
+// ---------------------------------------------------------------------------------------------
+template <bool FAST>
+__global__ void __launch_bounds__(256) indices3_kernel(AccParams p, int32_t* __restrict__ g0, int32_t* __restrict__ k) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  unsigned fb = 0;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += stride) {
+    bool live = true;
+    const Pre q = pre_part<FAST>(p, p.x[i], p.y[i], p.z[i], live);
+    Idx ix;
+    const bool ok = index_part<FAST>(p, q, p.vx[i], p.vy[i], p.vz[i], live, ix, fb);
+    g0[i] = ok ? ix.g0 : SIM_GATE_NONE;
+    k[i] = ok ? (ix.k & (p.N - 1)) : -1;
+  }
+  if (fb) atomicAdd(&p.counters[kCtrFallback], fb);
+}
+
+cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches) {
+  if (p.n == 0) return cudaSuccess;
+  const unsigned long long want = (p.n + 255) / 256;
+  const int grid = (int)(want < 148ull * 16 ? want : 148ull * 16);
+  if (p.index_path && p.fast_ok) indices3_kernel<true><<<grid, 256, 0, st>>>(p, g0, k);
+  else indices3_kernel<false><<<grid, 256, 0, st>>>(p, g0, k);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
 // Launchers
 // ---------------------------------------------------------------------------------------------
 typedef void (*W3Kernel)(AccParams);

@@ -34,8 +34,8 @@ __device__ __forceinline__ float cycles_fraction(double q) {
 // Returns (g0, k wrapped, bits of w1, bits of fr); g0 = SIM_GATE_NONE when the scatterer is dropped.
 // ---------------------------------------------------------------------------------------------
 struct CanonConsts {
-  double rg0, inv_dR, cD, two_over_lambda, fr0, svx, svy, svz;
-  int G, N;
+  double rg0, inv_dR, cD, two_over_lambda, fr0, svx, svy, svz, pri, cP;
+  int G, N, mode;
 };
 
 static __device__ __noinline__ int4 canonical_tail(CanonConsts c, double dx, double dy, double dz, float vxf,
@@ -50,8 +50,16 @@ static __device__ __noinline__ int4 canonical_tail(CanonConsts c, double dx, dou
   const double dvx = __dsub_rn((double)vxf, c.svx);
   const double dvy = __dsub_rn((double)vyf, c.svy);
   const double dvz = __dsub_rn((double)vzf, c.svz);
-  const double rdot = __ddiv_rn(__fma_rn(dvz, dz, __fma_rn(dvy, dy, __dmul_rn(dvx, dx))), R);
-  const double kf = __dmul_rn(rdot, c.cD);
+  double kf;
+  if (c.mode == SIM_DOPPLER_PULSE_PAIR) {
+    // Algorithm 1 lines 5-7: the offset one PRI later, R' - R, in bins (reading R4)
+    const double dx1 = __fma_rn(dvx, c.pri, dx), dy1 = __fma_rn(dvy, c.pri, dy), dz1 = __fma_rn(dvz, c.pri, dz);
+    const double R1 = __dsqrt_rn(__fma_rn(dz1, dz1, __fma_rn(dy1, dy1, __dmul_rn(dx1, dx1))));
+    kf = __dmul_rn(__dsub_rn(R1, R), c.cP);
+  } else {
+    const double rdot = __ddiv_rn(__fma_rn(dvz, dz, __fma_rn(dvy, dy, __dmul_rn(dvx, dx))), R);
+    kf = __dmul_rn(rdot, c.cD);
+  }
   if (!(fabs(kf) < 1073741824.0)) return dropped;
   const double kk = floor(__dadd_rn(kf, 0.5));
   // N is a power of two: two's-complement AND is the mathematical mod
@@ -65,6 +73,7 @@ __device__ __forceinline__ bool canonical(const AccParams& p, double dx, double 
   CanonConsts c;
   c.rg0 = p.rg0; c.inv_dR = p.inv_dR; c.cD = p.cD; c.two_over_lambda = p.two_over_lambda; c.fr0 = p.fr0;
   c.svx = p.svx; c.svy = p.svy; c.svz = p.svz; c.G = p.G; c.N = p.N;
+  c.pri = p.pri; c.cP = p.cP; c.mode = p.doppler_mode;
   const int4 r = canonical_tail(c, dx, dy, dz, vxf, vyf, vzf);
   if (r.x == SIM_GATE_NONE) return false;
   o.g0 = r.x;

@@ -50,6 +50,7 @@ const char* check_config(const sim_config* c) {
   if (c->pulses_per_update < 1) return "pulses_per_update must be >= 1";
   if (c->max_pending_updates < 2) return "max_pending_updates must be >= 2";
   if (c->weight_mode != SIM_W_SQRT && c->weight_mode != SIM_W_LINEAR) return "unknown weight_mode";
+  if (c->doppler_mode != SIM_DOPPLER_ANALYTIC && c->doppler_mode != SIM_DOPPLER_PULSE_PAIR) return "unknown doppler_mode";
   if (!(c->wavelength_m > 0) || !std::isfinite(c->wavelength_m)) return "wavelength_m must be > 0";
   if (!(c->prf_hz > 0) || !std::isfinite(c->prf_hz)) return "prf_hz must be > 0";
   if (!(c->gate_spacing_m > 0) || !std::isfinite(c->gate_spacing_m)) return "gate_spacing_m must be > 0";
@@ -284,7 +285,11 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.inv_dR = 1.0 / h->cfg.gate_spacing_m;
   p.two_over_lambda = 2.0 / h->cfg.wavelength_m;
   p.cD = (-2.0 * (double)h->cfg.n_doppler) / (h->cfg.wavelength_m * h->cfg.prf_hz);
+  p.doppler_mode = h->cfg.doppler_mode;
+  p.pri = 1.0 / h->cfg.prf_hz;
+  p.cP = (-2.0 * (double)h->cfg.n_doppler) / h->cfg.wavelength_m;
   fast_path_constants(h, sat, p);
+  if (p.doppler_mode == SIM_DOPPLER_PULSE_PAIR) p.fast_ok = 0;   // the polynomial path covers the analytic Doppler only
   const double bn = std::sqrt(sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
                               sat->boresight[2] * sat->boresight[2]);
   p.bx = (float)(sat->boresight[0] / bn);
@@ -656,7 +661,8 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   if (rc) return rc;
   AccParams p = make_acc_params(h, &s, sat, nullptr);
   int l = 0;
-  cudaError_t e = launch_indices(p, d_gate0, d_bin, h->stream, &l);
+  cudaError_t e = h->opt_variant >= 2 ? launch_indices3(p, d_gate0, d_bin, h->stream, &l)
+                                      : launch_indices(p, d_gate0, d_bin, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
   return SIM_OK;
@@ -668,6 +674,8 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
   switch (option) {
     case SIM_OPT_ACC_VARIANT:
       if (value > 3) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
+      if (value < 2 && h->cfg.doppler_mode == SIM_DOPPLER_PULSE_PAIR)
+        return fail(h, SIM_ERR_INVALID_ARG, "pulse-pair Doppler is implemented by accumulation variants 2 and 3 only");
       h->opt_variant = (int)value;
       variant_defaults(h);   // warps, per-lane count and epoch length are per variant: back to that variant's defaults
       if (value >= 2) {

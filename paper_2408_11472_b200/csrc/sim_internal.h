@@ -31,6 +31,8 @@ struct AccParams {
   double inv_dR;          // 1.0 / gate_spacing
   double two_over_lambda; // 2.0 / wavelength
   double cD;              // (-2.0 * N) / (wavelength * PRF)
+  double pri, cP;         // pulse-pair Doppler: 1.0 / PRF and (-2.0 * N) / wavelength
+  int doppler_mode;       // SIM_DOPPLER_*
   // ---- fast index path: delta = R - rg0 from u = R^2 - rg0^2 by series, no sqrt / div ----
   double rg0sq_hi, rg0sq_lo;  // rg0^2 as an exact double-double
   double u_lo, u_hi;          // u outside [u_lo, u_hi] is certainly outside the gate window
@@ -100,6 +102,8 @@ cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, i
 int acc_ws3_chunk(int ncw, int pt);
 cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
                            int* launches);
+// the index routine of the warp-specialised kernels (variants 2 and 3)
+cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches);
 size_t acc_tile_smem_bytes(int G, int W, int per_thread);
 cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);

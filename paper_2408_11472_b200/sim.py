@@ -17,6 +17,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_BAD_CONFIG, ERR_WORKSPACE, ERR_NOT_READY, ERR_OVERFLOW, ERR_CUDA = -1, -2, -3, -4, -5, -6
 W_SQRT, W_LINEAR = 0, 1
 ACC_APPEND = 1
+DOPPLER_ANALYTIC, DOPPLER_PULSE_PAIR = 0, 1
 SYN_FINAL = 1
 GATE_NONE = -(2**31)
 OPT_ACC_VARIANT, OPT_ACC_BLOCKS, OPT_ACC_SUPERCHUNK, OPT_ACC_WINDOW_BINS, OPT_GUARD_LSB, OPT_INDEX_PATH = 1, 2, 3, 4, 5, 6
@@ -41,7 +42,7 @@ class SimConfig(C.Structure):
     _fields_ = [
         ("struct_size", C.c_uint32), ("n_gates", C.c_int32), ("n_doppler", C.c_int32),
         ("pulses_per_update", C.c_int32), ("max_pending_updates", C.c_int32), ("weight_mode", C.c_int32),
-        ("device", C.c_int32), ("wavelength_m", C.c_double), ("prf_hz", C.c_double),
+        ("device", C.c_int32), ("doppler_mode", C.c_int32), ("wavelength_m", C.c_double), ("prf_hz", C.c_double),
         ("gate_spacing_m", C.c_double), ("antenna_alpha", C.c_double),
         ("host_stage_scatterers", C.c_int64), ("host_stage_pulses", C.c_int64),
     ]
@@ -102,9 +103,9 @@ def load_library(build_if_missing: bool = True):
 
 def make_config(n_gates, n_doppler, pulses_per_update, wavelength_m, prf_hz, gate_spacing_m,
                 antenna_alpha, max_pending_updates=4, weight_mode=W_SQRT, device=0,
-                host_stage_scatterers=0, host_stage_pulses=0) -> SimConfig:
+                host_stage_scatterers=0, host_stage_pulses=0, doppler_mode=DOPPLER_ANALYTIC) -> SimConfig:
     return SimConfig(C.sizeof(SimConfig), int(n_gates), int(n_doppler), int(pulses_per_update),
-                     int(max_pending_updates), int(weight_mode), int(device), float(wavelength_m),
+                     int(max_pending_updates), int(weight_mode), int(device), int(doppler_mode), float(wavelength_m),
                      float(prf_hz), float(gate_spacing_m), float(antenna_alpha),
                      int(host_stage_scatterers), int(host_stage_pulses))
 

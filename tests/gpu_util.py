@@ -28,9 +28,9 @@ def to_cuda(scat):
     return {k: v.cuda().contiguous() for k, v in scat.items()}
 
 
-def oracle_cfg(orc, wl, weight_mode=0):
+def oracle_cfg(orc, wl, weight_mode=0, doppler_mode=0):
     return orc.make_config(wl.n_gates, wl.n_doppler, wl.pulses_per_update, wl.wavelength_m, wl.prf_hz,
-                           wl.gate_spacing_m, wl.antenna_alpha, weight_mode)
+                           wl.gate_spacing_m, wl.antenna_alpha, weight_mode, doppler_mode)
 
 
 def oracle_sat(orc, wl, u):
@@ -38,8 +38,8 @@ def oracle_sat(orc, wl, u):
     return orc.make_sat(s["pos"], s["vel"], s["boresight"], s["range_gate0_m"])
 
 
-def oracle_spectra(orc, wl, scat_np, updates, weight_mode=0, nthreads=None):
-    cfg = oracle_cfg(orc, wl, weight_mode)
+def oracle_spectra(orc, wl, scat_np, updates, weight_mode=0, nthreads=None, doppler_mode=0):
+    cfg = oracle_cfg(orc, wl, weight_mode, doppler_mode)
     nthreads = nthreads or orc.max_threads()
     out = []
     for u in updates:

@@ -33,7 +33,8 @@ def test_header_symbols_are_exported(sim_mod):
 
 def test_struct_layout_matches_header(sim_mod):
     # sizes the C side checks through struct_size; offsets follow natural alignment
-    assert C.sizeof(sim_mod.SimConfig) == 4 * 7 + 4 + 8 * 4 + 8 * 2
+    assert C.sizeof(sim_mod.SimConfig) == 4 * 8 + 8 * 4 + 8 * 2
+    assert sim_mod.SimConfig.doppler_mode.offset == 28 and sim_mod.SimConfig.wavelength_m.offset == 32
     assert C.sizeof(sim_mod.SimScatterers) == 8 * 8
     assert C.sizeof(sim_mod.SimSatState) == 8 * 10
     assert C.sizeof(sim_mod.SimStats) == 8 * 4
