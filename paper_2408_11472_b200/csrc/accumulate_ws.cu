@@ -418,7 +418,7 @@ cudaError_t acc_ws_blocks_per_sm(int G, int W, int ncw, int stages, int* blocks)
 
 cudaError_t launch_accumulate_ws(const AccParams& p, int ncw, int blocks, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  WsKernel k = ws_kernel(ncw, p.index_path && p.fast_ok);
+  WsKernel k = ws_kernel(ncw, p.index_path && p.fast_ok && p.doppler_mode == SIM_DOPPLER_ANALYTIC);
   if (!k) return cudaErrorInvalidValue;
   const size_t smem = acc_ws_smem_bytes(p.G, p.W, ncw, p.stages);
   cudaError_t e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);

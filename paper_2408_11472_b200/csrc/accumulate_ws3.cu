@@ -101,7 +101,7 @@ struct Vec<4> {
   }
 };
 
-template <int NCW, int PT, int IL, bool FAST>
+template <int NCW, int PT, int IL, int MODE>
 __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 : 1)) acc_ws3_kernel(AccParams p) {
   constexpr int CH = NCW * 32 * PT;
   constexpr unsigned kStageBytes = 7u * CH * 4u;
@@ -257,7 +257,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
   #pragma unroll
         for (int j = 0; j < IL; ++j) {
           ok[j] = s0.v[gi + j] > 0.0f;   // s0dA <= 0 or NaN: dead
-          q[j] = pre_part<FAST>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ok[j]);
+          q[j] = pre_part<MODE>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ok[j]);
           any |= ok[j];
         }
         if (!__any_sync(kFull, any)) continue;   // warp-uniform: the whole warp is dark
@@ -267,7 +267,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
         any = false;
   #pragma unroll
         for (int j = 0; j < IL; ++j) {
-          ok[j] = index_part<FAST>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], fallbacks);
+          ok[j] = index_part<MODE>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], fallbacks);
           float A;
           c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
           ab[j] = __float_as_int(A);
@@ -376,19 +376,27 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
   if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
 }
 
+// Which index routine a launch uses: the polynomial path of the configured Doppler source when the host found
+// its error bounds covered by the guard band, else the canonical sequence everywhere.
+static int acc_index_mode(const AccParams& p) {
+  if (!p.index_path) return kIdxCanonical;
+  if (p.doppler_mode == SIM_DOPPLER_PULSE_PAIR) return p.pp_ok ? kIdxFastPulsePair : kIdxCanonical;
+  return p.fast_ok ? kIdxFast : kIdxCanonical;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Index-only kernel (parity pin P11, sim_debug_indices): the index routine of the production kernel
 // (pre_part + index_part of scatter_math.cuh), one scatterer per thread, s0dA not consulted.
 // ---------------------------------------------------------------------------------------------
-template <bool FAST>
+template <int MODE>
 __global__ void __launch_bounds__(256) indices3_kernel(AccParams p, int32_t* __restrict__ g0, int32_t* __restrict__ k) {
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   unsigned fb = 0;
   for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += stride) {
     bool live = true;
-    const Pre q = pre_part<FAST>(p, p.x[i], p.y[i], p.z[i], live);
+    const Pre q = pre_part<MODE>(p, p.x[i], p.y[i], p.z[i], live);
     Idx ix;
-    const bool ok = index_part<FAST>(p, q, p.vx[i], p.vy[i], p.vz[i], live, ix, fb);
+    const bool ok = index_part<MODE>(p, q, p.vx[i], p.vy[i], p.vz[i], live, ix, fb);
     g0[i] = ok ? ix.g0 : SIM_GATE_NONE;
     k[i] = ok ? (ix.k & (p.N - 1)) : -1;
   }
@@ -399,8 +407,11 @@ cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStr
   if (p.n == 0) return cudaSuccess;
   const unsigned long long want = (p.n + 255) / 256;
   const int grid = (int)(want < 148ull * 16 ? want : 148ull * 16);
-  if (p.index_path && p.fast_ok) indices3_kernel<true><<<grid, 256, 0, st>>>(p, g0, k);
-  else indices3_kernel<false><<<grid, 256, 0, st>>>(p, g0, k);
+  switch (acc_index_mode(p)) {
+    case kIdxFast: indices3_kernel<kIdxFast><<<grid, 256, 0, st>>>(p, g0, k); break;
+    case kIdxFastPulsePair: indices3_kernel<kIdxFastPulsePair><<<grid, 256, 0, st>>>(p, g0, k); break;
+    default: indices3_kernel<kIdxCanonical><<<grid, 256, 0, st>>>(p, g0, k); break;
+  }
   ++*launches;
   return cudaGetLastError();
 }
@@ -410,21 +421,24 @@ cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStr
 // ---------------------------------------------------------------------------------------------
 typedef void (*W3Kernel)(AccParams);
 
-static W3Kernel ws3_kernel(int ncw, int pt, int il, bool fast) {
+static W3Kernel ws3_kernel(int ncw, int pt, int il, int mode) {
 #define W3_CASE(NCW_, PT_, IL_) \
-  if (ncw == NCW_ && pt == PT_ && il == IL_) return fast ? acc_ws3_kernel<NCW_, PT_, IL_, true> : acc_ws3_kernel<NCW_, PT_, IL_, false>;
+  if (ncw == NCW_ && pt == PT_ && il == IL_)                                                  \
+    return mode == kIdxFast ? acc_ws3_kernel<NCW_, PT_, IL_, kIdxFast>                         \
+         : mode == kIdxFastPulsePair ? acc_ws3_kernel<NCW_, PT_, IL_, kIdxFastPulsePair>       \
+                                     : acc_ws3_kernel<NCW_, PT_, IL_, kIdxCanonical>;
   W3_CASE(8, 2, 2) W3_CASE(8, 4, 4) W3_CASE(8, 4, 2) W3_CASE(12, 2, 2) W3_CASE(16, 4, 2) W3_CASE(20, 4, 2)
 #undef W3_CASE
   return nullptr;
 }
 
-bool acc_ws3_supported(int ncw, int pt, int il) { return ws3_kernel(ncw, pt, il, true) != nullptr; }
+bool acc_ws3_supported(int ncw, int pt, int il) { return ws3_kernel(ncw, pt, il, kIdxFast) != nullptr; }
 
 cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks) {
   const size_t smem = acc_ws3_smem_bytes(G, W, ncw, pt, stages);
   *blocks = 1 << 30;
-  for (int fast = 0; fast < 2; ++fast) {
-    W3Kernel k = ws3_kernel(ncw, pt, il, fast != 0);
+  for (int mode = 0; mode < 3; ++mode) {
+    W3Kernel k = ws3_kernel(ncw, pt, il, mode);
     if (!k) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -438,7 +452,7 @@ cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int sta
 
 cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, int blocks, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  W3Kernel k = ws3_kernel(ncw, pt, il, p.index_path && p.fast_ok);
+  W3Kernel k = ws3_kernel(ncw, pt, il, acc_index_mode(p));
   if (!k) return cudaErrorInvalidValue;
   const size_t smem = acc_ws3_smem_bytes(p.G, p.W, ncw, pt, p.stages);
   cudaError_t e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);

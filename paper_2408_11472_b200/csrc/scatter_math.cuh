@@ -12,6 +12,10 @@ constexpr double kMagicFxHalf = 6442450944.5;    // the same + 0.5 (nearest-bin 
 constexpr double kMagicPhase = 402653184.0;      // 1.5 * 2^28: low word = round(q * 2^24)
 constexpr int kFxOne = 1 << kFracBits;
 
+// index routines: the canonical fp64 sequence for every scatterer, or a polynomial path (analytic Doppler /
+// pulse-pair Doppler) with the canonical sequence inside the guard band
+enum { kIdxCanonical = 0, kIdxFast = 1, kIdxFastPulsePair = 2 };
+
 // What the index part of one scatterer yields.
 struct Idx {
   int g0;      // gate of the lower half, in [-1, G-1]
@@ -85,8 +89,8 @@ __device__ __forceinline__ bool canonical(const AccParams& p, double dx, double 
 }
 
 // Steps A2-A4 in two parts, so that a warp whose scatterers all miss the window can stop after the first.
-//   FAST = false: the canonical sequence for every scatterer.
-//   FAST = true:  everything is a short polynomial in u = R^2 - rg0^2 (no sqrt, no divide):
+//   MODE = kIdxCanonical: the canonical sequence for every scatterer.
+//   MODE = kIdxFast, kIdxFastPulsePair:  everything is a short polynomial in u = R^2 - rg0^2 (no sqrt, no divide):
 //       gf = (R - rg0)/dR = u (g1 + u (g2 + u g3)),   kf = num cD / R = num (j0 + u (j1 + u j2)),
 //     gate and bin are read from 2^-20 fixed point; whenever a coordinate lies within `guard` of an
 //     integer boundary the canonical sequence decides (bit-exact indices).
@@ -96,14 +100,14 @@ struct Pre {
 
 // Offsets from the satellite and the window pre-test.  `live` in: the scatterer is a candidate (s0dA > 0);
 // out: it may land in the gate window.
-template <bool FAST>
+template <int MODE>
 __device__ __forceinline__ Pre pre_part(const AccParams& p, float xf, float yf, float zf, bool& live) {
   Pre q;
   q.dx = __dsub_rn((double)xf, p.sx);
   q.dy = __dsub_rn((double)yf, p.sy);
   q.dz = __dsub_rn((double)zf, p.sz);
   q.u = 0.0;
-  if (FAST) {
+  if (MODE != kIdxCanonical) {
     // the three squares cancel against -rg0^2; every rounding is <= ulp(rg0^2) ~ 1e-4 m^2 (<< guard)
     q.u = fma(q.dz, q.dz, fma(q.dy, q.dy, fma(q.dx, q.dx, p.neg_rg0sq)));
     live = live && (q.u >= p.uw_lo) && (q.u <= p.uw_hi);   // false: certainly outside the window (or NaN)
@@ -112,21 +116,32 @@ __device__ __forceinline__ Pre pre_part(const AccParams& p, float xf, float yf, 
 }
 
 // Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.
-template <bool FAST>
+template <int MODE>
 __device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
                                            bool live, Idx& o, unsigned& fallbacks) {
-  if (!FAST) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+  if (MODE == kIdxCanonical) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
   const double u = q.u;
   const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
   const int gfx = __double2loint(__dadd_rd(gf, kMagicFx));            // floor(gf * 2^20)
   const int gfrac = gfx & (kFxOne - 1);
   const double dvx = (double)vxf - p.svx, dvy = (double)vyf - p.svy, dvz = (double)vzf - p.svz;
   const double num = fma(dvz, q.dz, fma(dvy, q.dy, dvx * q.dx));
-  const double kf = num * fma(u, fma(u, p.j2, p.j1), p.j0);
+  double kf;
+  if (MODE == kIdxFastPulsePair) {
+    // R' - R = w / (R' + R) with w = R'^2 - R^2 = (2 num + |dv|^2 / PRF) / PRF, computed without cancellation, and
+    // R' + R = 2 rg0 + 2 (R - rg0) + (R' - R);  1 / (1 + e) = 1 - e + e^2 (e <= 1e-4)
+    const double dv2 = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
+    const double w = p.pri * fma(dv2, p.pri, num + num);
+    const double e = fma(w, p.inv_2rg0, gf * p.two_dR) * p.inv_2rg0;
+    kf = (w * p.cP_2rg0) * fma(e, e - 1.0, 1.0);
+  } else {
+    kf = num * fma(u, fma(u, p.j2, p.j1), p.j0);
+  }
   const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));        // floor((kf + 0.5) * 2^20)
   const int kfrac = kfx & (kFxOne - 1);
-  const unsigned span = (unsigned)(kFxOne - 2 * p.guard);
-  const bool near = ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - p.guard) >= span) |
+  const int gk = MODE == kIdxFastPulsePair ? p.guard_k : p.guard;   // pulse-pair: wider Doppler guard band
+  const unsigned span = (unsigned)(kFxOne - 2 * p.guard), span_k = (unsigned)(kFxOne - 2 * gk);
+  const bool near = ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) |
                     !(fabs(kf) < 1024.0);
   if (live && near) {  // rare: a coordinate sits in the guard band
     ++fallbacks;

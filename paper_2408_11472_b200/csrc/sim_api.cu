@@ -153,7 +153,9 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
   const double rg0 = sat->range_gate0_m, dR = h->cfg.gate_spacing_m, lam = h->cfg.wavelength_m;
   const int G = h->cfg.n_gates;
   p.guard = h->opt_guard;
+  p.guard_k = h->opt_guard;
   p.fast_ok = 0;
+  p.pp_ok = 0;
   {  // frac(rg0 * 2 / lambda) to ~1e-17 cycles: product split into rounded part + exact residual
     const double c = 2.0 / lam, q = rg0 * c, qe = std::fma(rg0, c, -q);
     p.fr0 = (q - std::floor(q)) + qe;
@@ -199,6 +201,22 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
     const double eg = 0.04 * x * x * x * x * rg0 / dR + 4.0 * std::ldexp(r2, -52) / (2.0 * rg0 * dR) + 1e-13 * (G + 2);
     const double ek = 1024.0 * (0.32 * x * x * x + 1e-14);
     if (!(gd >= 4.0 * eg && gd >= 4.0 * ek && phase_ok && G + 2 < 2048)) p.fast_ok = 0;
+  }
+  {  // pulse-pair fast path (scatter_math.cuh, kIdxFastPulsePair).  The canonical R' - R carries the rounding of
+     // two square roots of ~rmax (each within 2 ulp of the exact root): up to 4 * 2^-53 * rmax * 2N / lambda bins of
+     // noise that the (accurate) fast value does not share; the Doppler guard band is 1.5 x that bound.  Series and
+     // roundings of the fast value itself: 1024 * (e^3 + 1e-14), e <= 2.2 emax.
+    const double cP_abs = 2.0 * (double)h->cfg.n_doppler / lam;
+    const double noise = 4.0 * std::ldexp(rmax, -53) * cP_abs;
+    const double x = 2.2 * emax;
+    const double own = 1024.0 * (x * x * x + 1e-14);
+    const double need = 1.5 * noise + 4.0 * own;
+    int gk = (int)std::ceil(need * (double)(1 << kFracBits));
+    if (gk < p.guard) gk = p.guard;
+    p.two_dR = 2.0 * dR;
+    p.cP_2rg0 = p.cP * p.inv_2rg0;
+    p.pp_ok = (p.fast_ok && gk <= (1 << (kFracBits - 3))) ? 1 : 0;   // the gate half of the bound is the analytic one
+    p.guard_k = h->cfg.doppler_mode == SIM_DOPPLER_PULSE_PAIR ? gk : p.guard;
   }
   // fp32 pre-test: |u_f32 - u| <= 2^-21 R^2 (three squares, two sums, the split satellite position and
   // rg0^2 each rounded to 2^-24); the margin is twice that at the far edge of the window
@@ -289,7 +307,6 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.pri = 1.0 / h->cfg.prf_hz;
   p.cP = (-2.0 * (double)h->cfg.n_doppler) / h->cfg.wavelength_m;
   fast_path_constants(h, sat, p);
-  if (p.doppler_mode == SIM_DOPPLER_PULSE_PAIR) p.fast_ok = 0;   // the polynomial path covers the analytic Doppler only
   const double bn = std::sqrt(sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
                               sat->boresight[2] * sat->boresight[2]);
   p.bx = (float)(sat->boresight[0] / bn);

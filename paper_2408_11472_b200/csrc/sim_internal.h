@@ -41,7 +41,10 @@ struct AccParams {
   double inv_rg0;             // 1 / rg0
   double fr0;                 // frac(rg0 * 2 / lambda), exact to ~1e-17
   int guard;                  // guard band in units of 2^-kFracBits around integer gate / bin boundaries
-  int fast_ok;                // host-side validity of the fast path for this geometry
+  int guard_k;                // the same for the Doppler coordinate (wider for the pulse-pair path)
+  int fast_ok;                // host-side validity of the fast path for this geometry (analytic Doppler)
+  int pp_ok;                  // ... of the pulse-pair fast path
+  double two_dR, cP_2rg0;     // pulse-pair fast path: 2 * gate_spacing, cP / (2 rg0)
   // ---- fp32 amplitude path ----
   float sxh, sxl, syh, syl, szh, szl;  // satellite position as float hi + lo
   float bx, by, bz;                    // unit boresight

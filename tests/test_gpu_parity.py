@@ -421,6 +421,15 @@ def test_pulse_pair_doppler(oracle, sim_mod, name):
     sim = sim_mod.Sim(sim_mod.config_for(wl, doppler_mode=sim_mod.DOPPLER_PULSE_PAIR))
     with pytest.raises(sim_mod.SimError):
         sim.set_option(sim_mod.OPT_ACC_VARIANT, 1)                 # variants 0 and 1 do not implement it
+    # polynomial path + guard band (default) against the canonical sequence everywhere: same bins, and the
+    # guard band stays thin although it is wider than the analytic one (it covers the cancellation noise of R' - R)
+    sim.read_counters(reset=True)
+    g0, k = sim.debug_indices(scat_cuda, sim_mod.sat_for(wl, 0))
+    fb = sim.read_counters(reset=True)["index_fallbacks"]
+    assert np.array_equal(k.cpu().numpy(), kp) and 0 < fb < 2e-3 * wl.n_scatterers
+    sim.set_option(sim_mod.OPT_INDEX_PATH, 0)
+    g0c, kc = sim.debug_indices(scat_cuda, sim_mod.sat_for(wl, 0))
+    assert torch.equal(g0, g0c) and torch.equal(k, kc) and sim.read_counters()["index_fallbacks"] == 0
 
 
 def test_maximum_sizes(oracle, sim_mod):
