@@ -21,6 +21,9 @@
  *                            "Summing the weighted time-long signals in the corresponding cells of Y"
  *                            (PAPER.md:100-101); eq. (1) at PAPER.md:61, W_i(x) = (1 - |i-x|/n_fast)^(1/2).
  *
+ *   R   oracle_regular    -- the REGULAR mode: per-pulse complex sum of all scatterers per
+ *                            range gate, surface "updated at each PRF" (reading R5).
+ *
  * Pins: every function here is pinned by tests/test_oracle_pins.py (closed forms, numpy.fft
  * special case, Parseval, brute-force regular-mode sum, an independent numpy restatement); the
  * pulse-pair Doppler mode by tests/test_oracle_pulse_pair.py (the literal arg(C_{i+1} C_i^*) estimator at
@@ -339,6 +342,84 @@ int oracle_synthesize(const oracle_config *c, int32_t n_spectra, const double *T
   }
   free(ysig);
   return 0;
+}
+
+/* REGULAR MODE: "the surface [is] updated at each PRF" and the raw
+ * data of a pulse are "obtained by summing the complex contributions from all the facets ... in each range
+ * gate".  Point scatterers and satellite in uniform motion from the states given at pulse 0 (reading R5):
+ * for pulse j (any sign), t_j = j / PRF, d_j = d + (v_p - v_sat) t_j, R_j = |d_j|, the two-gate linear split
+ * (A8) and the complex amplitude of step O1 evaluated at R_j, d_j; no Doppler axis.
+ * Y: [n_pulses][G] complex128 for pulses j0 .. j0 + n_pulses - 1; accumulate != 0 adds to Y. */
+static void regular_range(const oracle_config *c, const oracle_sat *s, int64_t lo, int64_t hi,
+                          const float *x, const float *y, const float *z, const float *vx,
+                          const float *vy, const float *vz, const float *s0dA, int64_t j0,
+                          int64_t n_pulses, double *Y) {
+  double inv_dR, two_over_lambda, cD, b[3];
+  constants(c, &inv_dR, &two_over_lambda, &cD);
+  unit_boresight(s, b);
+  const int G = c->n_gates;
+  for (int64_t p = lo; p < hi; ++p) {
+    if (!(s0dA[p] > 0.0f)) continue;
+    const double dx0 = (double)x[p] - s->pos[0], dy0 = (double)y[p] - s->pos[1], dz0 = (double)z[p] - s->pos[2];
+    const double dvx = (double)vx[p] - s->vel[0], dvy = (double)vy[p] - s->vel[1], dvz = (double)vz[p] - s->vel[2];
+    const double amp0 = sqrt((double)s0dA[p]);
+    for (int64_t jj = 0; jj < n_pulses; ++jj) {
+      const double t = (double)(j0 + jj) / c->prf_hz;
+      const double dx = fma(dvx, t, dx0), dy = fma(dvy, t, dy0), dz = fma(dvz, t, dz0);
+      const double R2 = fma(dz, dz, fma(dy, dy, dx * dx));
+      const double R = sqrt(R2);
+      const double gf = (R - s->range_gate0_m) * inv_dR;
+      if (!(gf >= -1.0 && gf < (double)G)) continue;
+      const double g0d = floor(gf);
+      const int g0 = (int)g0d;
+      const double w1 = gf - g0d, w0 = 1.0 - w1;
+      const double q = R * two_over_lambda;
+      const double fr = q - floor(q);
+      const double cx = dy * b[2] - dz * b[1], cy = dz * b[0] - dx * b[2], cz = dx * b[1] - dy * b[0];
+      const double sin2 = (cx * cx + cy * cy + cz * cz) / R2;
+      const double A = amp0 * exp(-c->antenna_alpha * sin2) / R2;
+      const double re = A * cos(TWO_PI * fr), im = -A * sin(TWO_PI * fr);
+      double *row = Y + (size_t)jj * G * 2;
+      if (g0 >= 0 && g0 < G) {
+        row[2 * g0] += w0 * re;
+        row[2 * g0 + 1] += w0 * im;
+      }
+      if (g0 + 1 >= 0 && g0 + 1 < G) {
+        row[2 * (g0 + 1)] += w1 * re;
+        row[2 * (g0 + 1) + 1] += w1 * im;
+      }
+    }
+  }
+}
+
+int oracle_regular(const oracle_config *c, const oracle_sat *s, int64_t n, const float *x, const float *y,
+                   const float *z, const float *vx, const float *vy, const float *vz, const float *s0dA,
+                   int64_t j0, int64_t n_pulses, double *Y, int accumulate, int nthreads) {
+  if (!c || !s || !Y || n < 0 || n_pulses < 0 || c->n_gates < 1) return -1;
+  const int64_t cells = n_pulses * c->n_gates;
+  if (!accumulate) memset(Y, 0, (size_t)cells * 2 * sizeof(double));
+  if (nthreads <= 1) {
+    regular_range(c, s, 0, n, x, y, z, vx, vy, vz, s0dA, j0, n_pulses, Y);
+    return 1;
+  }
+#ifdef _OPENMP
+  double *priv = (double *)calloc((size_t)nthreads * (size_t)cells * 2, sizeof(double));
+  if (!priv) return -2;
+#pragma omp parallel num_threads(nthreads)
+  {
+    const int t = omp_get_thread_num();
+    const int nt = omp_get_num_threads();
+    regular_range(c, s, n * t / nt, n * (t + 1) / nt, x, y, z, vx, vy, vz, s0dA, j0, n_pulses,
+                  priv + (size_t)t * cells * 2);
+  }
+  for (int t = 0; t < nthreads; ++t)
+    for (int64_t j = 0; j < cells * 2; ++j) Y[j] += priv[(size_t)t * cells * 2 + j];
+  free(priv);
+  return nthreads;
+#else
+  regular_range(c, s, 0, n, x, y, z, vx, vy, vz, s0dA, j0, n_pulses, Y);
+  return 1;
+#endif
 }
 
 int oracle_max_threads(void) {

@@ -75,6 +75,9 @@ def lib():
         L.oracle_doppler_coordinate.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
                                                 fp, fp, fp, fp, fp, fp, dp]
         L.oracle_doppler_coordinate.restype = C.c_int
+        L.oracle_regular.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
+                                     fp, fp, fp, fp, fp, fp, fp, C.c_int64, C.c_int64, dp, C.c_int, C.c_int]
+        L.oracle_regular.restype = C.c_int
         L.oracle_idft.argtypes = [C.c_int32, C.c_int32, dp, dp]
         L.oracle_idft.restype = C.c_int
         L.oracle_weight.argtypes = [C.c_int32, C.c_int32, C.c_int64]
@@ -154,6 +157,18 @@ def doppler_coordinate(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz):
     if rc < 0:
         raise RuntimeError(f"oracle_doppler_coordinate failed: {rc}")
     return kf
+
+
+def regular(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz, s0dA, j0, n_pulses, nthreads=1):
+    """Regular mode: [n_pulses][G] complex128 for pulses j0..j0+n_pulses-1 relative to the instant of `sat`."""
+    arrs = [_f32(a) for a in (x, y, z, vx, vy, vz, s0dA)]
+    n = arrs[0][0].size
+    Y = np.zeros((int(n_pulses), cfg.n_gates), dtype=np.complex128)
+    rc = lib().oracle_regular(C.byref(cfg), C.byref(sat), n, *[a[1] for a in arrs], int(j0), int(n_pulses),
+                              Y.ctypes.data_as(C.POINTER(C.c_double)), 0, int(nthreads))
+    if rc < 0:
+        raise RuntimeError(f"oracle_regular failed: {rc}")
+    return Y
 
 
 def idft(T):
