@@ -156,6 +156,18 @@ int sim_get_spectrum(sim_handle* h, int64_t update_index, void* d_out);
  * all-reduce partial spectra across GPUs in place). */
 int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset);
 
+/* REGULAR MODE (reading R5): the at-scale truth the fast mode
+ * approximates.  Scatterers (DEVICE arrays) and satellite are in uniform motion from the states given for pulse 0;
+ * for each pulse j = first_pulse .. first_pulse + n_pulses - 1 (any sign), at t_j = j / PRF, every scatterer's
+ * complex amplitude sqrt(s0dA) G(theta) / R^2 exp(-i 4 pi R / lambda) at ITS RANGE AT t_j is summed into its two
+ * gates (the linear split of step A3).  d_iq: DEVICE complex64 [n_pulses][G], gate fastest, 16-byte aligned.
+ * flags = 0: d_iq is zeroed first; SIM_ACC_APPEND: the sums are added to it (scenes delivered in pieces).
+ * Work is scatterers x pulses.  Independent of the spectra ring and of sim_synthesize_pulses.
+ * Errors: SIM_ERR_INVALID_ARG (NULL / misaligned), SIM_ERR_BAD_CONFIG (n_gates > ~768, or a gate window too
+ * deep for the polynomial gate coordinate). */
+int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat,
+                       int64_t first_pulse, int64_t n_pulses, void* d_iq, uint32_t flags);
+
 /* Runs the production index computation only: for each scatterer the gate g0 = floor(gf) in
  * [-1, G-1] and the Doppler bin k in [0, N); dropped scatterers give (SIM_GATE_NONE, -1).
  * d_gate0, d_bin: DEVICE int32[n].  Must match the canonical fp64 sequence bit for bit. */

@@ -621,6 +621,35 @@ int sim_synthesize_pulses_host(sim_handle* h, int64_t n_pulses, void* h_iq, uint
   return SIM_OK;
 }
 
+int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, int64_t first_pulse,
+                       int64_t n_pulses, void* d_iq, uint32_t flags) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (flags & ~SIM_ACC_APPEND) return fail(h, SIM_ERR_INVALID_ARG, "unknown regular-mode flag");
+  if (n_pulses < 0 || n_pulses > (1 << 24)) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses outside 0..2^24");
+  if (first_pulse < -(1LL << 40) || first_pulse > (1LL << 40)) return fail(h, SIM_ERR_INVALID_ARG, "first_pulse out of range");
+  int rc = check_scatterers(h, d_scat, true);
+  if (rc) return rc;
+  rc = check_sat(h, sat);
+  if (rc) return rc;
+  if (n_pulses == 0) return SIM_OK;
+  if (!d_iq) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer is NULL");
+  if (misaligned(d_iq)) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer must be 16-byte aligned");
+  AccParams p = make_acc_params(h, d_scat, sat, nullptr);
+  if (!p.fast_ok) return fail(h, SIM_ERR_BAD_CONFIG, "regular mode: gate window outside the range of the polynomial gate coordinate");
+  cudaError_t e = cudaSuccess;
+  if (!(flags & SIM_ACC_APPEND)) {
+    e = cudaMemsetAsync(d_iq, 0, (size_t)n_pulses * h->cfg.n_gates * sizeof(float2), h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(regular iq)");
+  }
+  int l = 0;
+  e = launch_regular(p, static_cast<float2*>(d_iq), first_pulse, (int)n_pulses, h->cfg.prf_hz, h->sm_count, h->smem_optin,
+                     h->stream, &l);
+  h->launches += l;
+  if (e == cudaErrorInvalidConfiguration) return fail(h, SIM_ERR_BAD_CONFIG, "regular mode: n_gates too large for one pulse row per thread in shared memory");
+  if (e != cudaSuccess) return cuda_fail(h, e, "regular-mode launch");
+  return SIM_OK;
+}
+
 int sim_synchronize(sim_handle* h) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   cudaError_t e = cudaStreamSynchronize(h->stream);

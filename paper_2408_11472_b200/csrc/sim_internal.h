@@ -109,6 +109,10 @@ cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStre
 cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches);
 size_t acc_tile_smem_bytes(int G, int W, int per_thread);
 cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks);
+// regular mode (regular.cu): Y[n_pulses][G] += per-pulse coherent sums; cudaErrorInvalidConfiguration when G is too
+// large for one pulse row per thread in shared memory
+cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,
+                           size_t smem_optin, cudaStream_t st, int* launches);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
 int synth_gate_tile(int N, int G, long long n_segments, int sm_count);

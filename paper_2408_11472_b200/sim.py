@@ -28,7 +28,7 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",
     "sim_accumulate_update_host", "sim_synthesize_pulses_host", "sim_synchronize", "sim_destroy",
     "sim_get_spectrum", "sim_spectrum_offset", "sim_debug_indices", "sim_set_option", "sim_get_stats",
-    "sim_read_counters", "sim_last_error",
+    "sim_read_counters", "sim_last_error", "sim_regular_pulses",
 ]
 
 
@@ -183,6 +183,20 @@ class Sim:
         if out.dtype != torch.complex64 or not out.is_contiguous() or out.numel() < n_pulses * G or not out.is_cuda:
             raise ValueError("out must be a contiguous CUDA complex64 tensor of at least n_pulses*G elements")
         self._check(self.lib.sim_synthesize_pulses(self._h, n_pulses, out.data_ptr(), flags), self._h)
+        return out
+
+    def regular_pulses(self, scat: dict, sat: SimSatState, first_pulse: int, n_pulses: int,
+                       out: "torch.Tensor | None" = None, flags: int = 0):
+        """Regular mode (sim_regular_pulses): [n_pulses][G] complex64 for pulses first_pulse.. relative to `sat`."""
+        G = self.cfg.n_gates
+        if out is None:
+            out = torch.empty((n_pulses, G), dtype=torch.complex64, device=self.device)
+        if out.dtype != torch.complex64 or not out.is_contiguous() or out.numel() < n_pulses * G or not out.is_cuda:
+            raise ValueError("out must be a contiguous CUDA complex64 tensor of at least n_pulses*G elements")
+        s = _scat_struct(scat, cuda=True)
+        self._check(self.lib.sim_regular_pulses(self._h, C.byref(s), C.byref(sat), C.c_int64(first_pulse),
+                                                C.c_int64(n_pulses), C.c_void_p(out.data_ptr()), C.c_uint32(flags)),
+                    self._h)
         return out
 
     def accumulate_update_host(self, scat: dict, sat: SimSatState, flags: int = 0):

@@ -432,6 +432,53 @@ def test_pulse_pair_doppler(oracle, sim_mod, name):
     assert torch.equal(g0, g0c) and torch.equal(k, kc) and sim.read_counters()["index_fallbacks"] == 0
 
 
+# ---- regular mode ---------------------------------------------
+REG_CASES = {
+    # (workload, first pulse, pulses): several pulse tiles and scatterer slices, ragged sizes, negative pulses
+    "nadir": (W.get("nadir_patch_16m").scaled(n_along=300, n_cross=333, n_updates=1), -37, 300),
+    "sar_pm_coarse": (W.get("sar_footprint_268m").scaled(n_along=256, n_cross=256, spacing_m=64.0, n_updates=1), 0, 97),
+    "tiny_g64": (W.get("tiny").scaled(n_along=128, n_cross=130), 1000, 64),
+}
+
+
+@pytest.mark.parametrize("name", sorted(REG_CASES))
+def test_regular_mode(oracle, sim_mod, name):
+    wl, j0, npul = REG_CASES[name]
+    scat = W.scatterers(wl)
+    scat["s0dA"][5:40] = 0.0                                       # dead scatterers
+    scat["z"][100:130] = 200.0                                     # out of the window at every pulse
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    Y_ref = oracle.regular(U.oracle_cfg(oracle, wl), U.oracle_sat(oracle, wl, 0), *[scat_np[f] for f in W.FIELDS],
+                           j0, npul, nthreads=oracle.max_threads())
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    Y = sim.regular_pulses(scat_cuda, sim_mod.sat_for(wl, 0), j0, npul).cpu().numpy()
+    for lo in range(0, npul, 64):                                   # per block of <= 64 pulses, like an IQ block
+        e = U.rel_l2(Y[lo:lo + 64], Y_ref[lo:lo + 64])
+        assert e <= U.TOL, (name, lo, e)
+    # two halves of the scene with SIM_ACC_APPEND equal one call (linearity; the paper's tiles)
+    n = wl.n_scatterers // 2 // 4 * 4
+    a = {k: v[:n] for k, v in scat_cuda.items()}
+    b = {k: v[n:] for k, v in scat_cuda.items()}
+    Y2 = sim.regular_pulses(a, sim_mod.sat_for(wl, 0), j0, npul)
+    sim.regular_pulses(b, sim_mod.sat_for(wl, 0), j0, npul, out=Y2, flags=sim_mod.ACC_APPEND)
+    assert U.rel_l2(Y2.cpu().numpy(), Y_ref) <= U.TOL
+    # pulse 0 of the regular mode is the update pulse of the fast mode (reading A2, pin P7)
+    sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+    T = sim.get_spectrum(0).cpu().numpy()
+    Y0 = sim.regular_pulses(scat_cuda, sim_mod.sat_for(wl, 0), 0, 1).cpu().numpy()[0]
+    assert U.rel_l2(T.sum(axis=1), Y0) <= U.TOL
+
+
+def test_regular_mode_errors(sim_mod):
+    wl = W.get("tiny").scaled(n_gates=1024, gate_spacing_m=0.05)
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    scat = U.to_cuda({k: v[:4096] for k, v in W.scatterers(wl).items()})
+    with pytest.raises(sim_mod.SimError) as ei:
+        sim.regular_pulses(scat, sim_mod.sat_for(wl, 0), 0, 16)    # one 1024-gate row per thread does not fit
+    assert ei.value.code == sim_mod.ERR_BAD_CONFIG
+    assert sim.regular_pulses(scat, sim_mod.sat_for(wl, 0), 0, 0).numel() == 0
+
+
 def test_maximum_sizes(oracle, sim_mod):
     wl = W.get("tiny").scaled(n_along=256, n_cross=256, n_gates=1024, n_doppler=1024, pulses_per_update=1024,
                               n_updates=2, gate_spacing_m=0.05)
