@@ -265,13 +265,41 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
         float2 c[IL];
         int ab[IL];
         any = false;
+        if (MODE == kIdxCanonical) {
   #pragma unroll
-        for (int j = 0; j < IL; ++j) {
-          ok[j] = index_part<MODE>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], fallbacks);
-          float A;
-          c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
-          ab[j] = __float_as_int(A);
-          any |= ok[j];
+          for (int j = 0; j < IL; ++j) {
+            ok[j] = index_part<MODE>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], fallbacks);
+            float A;
+            c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
+            ab[j] = __float_as_int(A);
+            any |= ok[j];
+          }
+        } else {
+          // polynomial path straight through for all IL scatterers (no call site in the hot flow: calls cut the live
+          // ranges of the constants), then ONE cold patch-up for the rare guard-band cases
+          bool near[IL], any_near = false;
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) {
+            ok[j] = index_fast<MODE>(p, q[j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ok[j], ix[j], near[j]);
+            float A;
+            c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
+            ab[j] = __float_as_int(A);
+            any_near |= near[j];
+          }
+          if (__any_sync(kFull, any_near)) {
+  #pragma unroll
+            for (int j = 0; j < IL; ++j) {
+              if (near[j]) {
+                ++fallbacks;
+                ok[j] = canonical(p, q[j].dx, q[j].dy, q[j].dz, vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ix[j]);
+                float A;
+                c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
+                ab[j] = __float_as_int(A);
+              }
+            }
+          }
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) any |= ok[j];
         }
         const unsigned okm = __ballot_sync(kFull, any);
         if (okm == 0) continue;

@@ -115,11 +115,12 @@ __device__ __forceinline__ Pre pre_part(const AccParams& p, float xf, float yf, 
   return q;
 }
 
-// Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.
+// The polynomial index path WITHOUT the guard-band call: fills `o` and sets `near` when a coordinate lies in the
+// guard band (the caller then lets the canonical sequence decide; until then `o` is not trustworthy).
+// MODE = kIdxFast or kIdxFastPulsePair.  Returns `live`.
 template <int MODE>
-__device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
-                                           bool live, Idx& o, unsigned& fallbacks) {
-  if (MODE == kIdxCanonical) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+__device__ __forceinline__ bool index_fast(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
+                                           bool live, Idx& o, bool& near) {
   const double u = q.u;
   const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
   const int gfx = __double2loint(__dadd_rd(gf, kMagicFx));            // floor(gf * 2^20)
@@ -141,17 +142,26 @@ __device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, flo
   const int kfrac = kfx & (kFxOne - 1);
   const int gk = MODE == kIdxFastPulsePair ? p.guard_k : p.guard;   // pulse-pair: wider Doppler guard band
   const unsigned span = (unsigned)(kFxOne - 2 * p.guard), span_k = (unsigned)(kFxOne - 2 * gk);
-  const bool near = ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) |
-                    !(fabs(kf) < 1024.0);
-  if (live && near) {  // rare: a coordinate sits in the guard band
-    ++fallbacks;
-    return canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
-  }
+  near = live && (((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) | !(fabs(kf) < 1024.0));
   o.g0 = gfx >> kFracBits;
   o.k = kfx >> kFracBits;
   o.w1 = (float)gfrac * p.w_scale;
   o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
   o.gfx = (float)gfx;
+  return live;
+}
+
+// Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.
+template <int MODE>
+__device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
+                                           bool live, Idx& o, unsigned& fallbacks) {
+  if (MODE == kIdxCanonical) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+  bool near;
+  live = index_fast<MODE>(p, q, vxf, vyf, vzf, live, o, near);
+  if (near) {  // rare: a coordinate sits in the guard band
+    ++fallbacks;
+    return canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
+  }
   return live;
 }
 
