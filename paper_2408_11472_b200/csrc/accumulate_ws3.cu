@@ -171,15 +171,29 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
         const int r0 = max(sh::ld(slot + 4 * kS3Gmin), 0), r1 = min(sh::ld(slot + 4 * kS3Gmax) + 1, G - 1);
         const int ncell = (r1 >= r0) ? (r1 - r0 + 1) << logW : 0;   // nothing fitted (all escaped): empty range
         const unsigned tile = tile0 + b * tile_bytes;
-        for (int cc = lane; cc < ncell; cc += 32) {
-          const int r = r0 + (cc >> logW), kw = cc & (Wp - 1);
-          if (kw >= W) continue;
-          const unsigned a = tile + 4u * (unsigned)((r + 1) * RS + kw);
-          const int re = sh::ld(a), im = sh::ld(a + plane_bytes);
-          if (re | im) {
-            sh::st(a, 0);
-            sh::st(a + plane_bytes, 0);
-            atomicAdd(&p.T[(size_t)r * N + ((k0 + kw) & (N - 1))], make_float2((float)re * inv_s, (float)im * inv_s));
+        // four cells per lane per pass, their eight loads in flight together: the drain must be well under one
+        // epoch long or the compute warps wait for their tile (profiles/r01_v3_final.md)
+        for (int cc0 = lane; cc0 < ncell; cc0 += 128) {
+          int re[4], im[4];
+          unsigned a[4];
+  #pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int cc = cc0 + 32 * u;
+            const int r = r0 + (cc >> logW), kw = cc & (Wp - 1);
+            const bool v = cc < ncell && kw < W;
+            a[u] = tile + 4u * (unsigned)((r + 1) * RS + kw);
+            re[u] = v ? sh::ld(a[u]) : 0;
+            im[u] = v ? sh::ld(a[u] + plane_bytes) : 0;
+          }
+  #pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (re[u] | im[u]) {
+              const int cc = cc0 + 32 * u;
+              const int r = r0 + (cc >> logW), kw = cc & (Wp - 1);
+              sh::st(a[u], 0);
+              sh::st(a[u] + plane_bytes, 0);
+              atomicAdd(&p.T[(size_t)r * N + ((k0 + kw) & (N - 1))], make_float2((float)re[u] * inv_s, (float)im[u] * inv_s));
+            }
           }
         }
         __syncwarp();
