@@ -54,14 +54,31 @@ __global__ void regular_kernel(RegParams rp) {
 
   const unsigned long long per = (p.n + rp.n_slices - 1) / rp.n_slices;
   const unsigned long long lo = per * blockIdx.y, hi = (lo + per < p.n) ? lo + per : p.n;
+  // Each thread prepares up to kPrep scatterers of a chunk.  Their raw inputs are fetched into registers one chunk
+  // ahead, so that the global-load latency is hidden behind the evaluation of the current chunk.
+  constexpr int kPrep = (kRegChunk + 31) / 32;   // enough for the smallest block (32 threads)
+  float in[kPrep][7];
+  auto fetch = [&](unsigned long long base) {
+#pragma unroll
+    for (int k = 0; k < kPrep; ++k) {
+      const unsigned long long q = base + tid + (unsigned long long)k * JT;
+      const bool v = tid + k * JT < kRegChunk && q < hi;
+      in[k][0] = v ? p.x[q] : 0.0f; in[k][1] = v ? p.y[q] : 0.0f; in[k][2] = v ? p.z[q] : 0.0f;
+      in[k][3] = v ? p.vx[q] : 0.0f; in[k][4] = v ? p.vy[q] : 0.0f; in[k][5] = v ? p.vz[q] : 0.0f;
+      in[k][6] = v ? p.s0dA[q] : 0.0f;
+    }
+  };
+  if (lo < hi) fetch(lo);
   for (unsigned long long base = lo; base < hi; base += kRegChunk) {
     const int m = (int)((hi - base < (unsigned long long)kRegChunk) ? hi - base : kRegChunk);
     __syncthreads();   // the previous chunk has been consumed
-    for (int i = tid; i < m; i += JT) {
-      const unsigned long long q = base + i;
-      const float s0 = p.s0dA[q];
-      const double dx = __dsub_rn((double)p.x[q], p.sx), dy = __dsub_rn((double)p.y[q], p.sy), dz = __dsub_rn((double)p.z[q], p.sz);
-      const double dvx = (double)p.vx[q] - p.svx, dvy = (double)p.vy[q] - p.svy, dvz = (double)p.vz[q] - p.svz;
+#pragma unroll
+    for (int k = 0; k < kPrep; ++k) {
+      const int i = tid + k * JT;
+      if (i >= m) continue;
+      const float s0 = in[k][6];
+      const double dx = __dsub_rn((double)in[k][0], p.sx), dy = __dsub_rn((double)in[k][1], p.sy), dz = __dsub_rn((double)in[k][2], p.sz);
+      const double dvx = (double)in[k][3] - p.svx, dvy = (double)in[k][4] - p.svy, dvz = (double)in[k][5] - p.svz;
       s_u0[i] = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.neg_rg0sq)));
       s_a[i] = 2.0 * fma(dvz, dz, fma(dvy, dy, dvx * dx));
       s_b[i] = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
@@ -72,6 +89,7 @@ __global__ void regular_kernel(RegParams rp) {
       s_amp[i] = (s0 > 0.0f) ? sqrt_approx(s0) : 0.0f;   // s0dA <= 0 or NaN: contributes nothing
     }
     __syncthreads();
+    if (base + kRegChunk < hi) fetch(base + kRegChunk);   // in flight during the evaluation below
     if (!pulse_ok) continue;
 #pragma unroll 2
     for (int i = 0; i < m; ++i) {
