@@ -354,17 +354,24 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   unsigned long long unit = kAccChunk;
   if (h->opt_variant >= 2) {
     const int ch = h->opt_variant == 3 ? acc_ws3_chunk(h->opt_ncw, h->opt_pt) : acc_ws_chunk(h->opt_ncw);
+    // chunks per fixed-point epoch: as many as the epoch length allows, but a small input is cut into enough
+    // scheduling units (whole epochs) to give every resident block some work
+    int ec = h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1;
+    if (h->opt_variant == 3) {
+      const unsigned long long fair = s->n / ((unsigned long long)ch * (unsigned long long)blocks * 2ull);
+      if (fair < (unsigned long long)ec) ec = fair > 0 ? (int)fair : 1;
+    }
     p.W = h->ws_W;
     p.stages = h->ws_stages;
     p.wait_hint = (unsigned)h->opt_wait_hint;
     {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
-      const int L = (h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1) * ch;
+      const int L = ec * ch;
       int lg = 0;
       while ((1 << lg) < L + 1) ++lg;
       p.fx_cap = 31 - lg;
       p.fx_target = p.fx_cap - 2 < 16 ? p.fx_cap - 2 : 16;
     }
-    p.epoch_chunks = h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1;
+    p.epoch_chunks = ec;
     unit = (unsigned long long)ch * p.epoch_chunks;     // super-chunk = whole epochs: a jump never splits one
   }
   sc = (sc + unit - 1) / unit * unit;
