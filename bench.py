@@ -346,7 +346,8 @@ def main():
             "metric": "scatterers accumulated + IQ synthesised per second (whole step)",
             "value": value, "unit": "scatterers/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": "f32 accumulate / f64 index+phase", "data": "synthetic",
+            "dtype": "f32", "dtype_note": "fp32 amplitudes, accumulation (block-floating int32 tiles) and FFT; fp64 range, gate/bin index and phase reduction",
+            "data": "synthetic",
             "config": {"workload": wl.name, "scatterers": wl.n_scatterers, "gates": G, "doppler_bins": N,
                        "pulses_per_update": P, "updates": U, "l2": "inputs larger than L2 (no flush needed)"
                        if BYTES_PER_SCATTERER * n_local > 2.5e8 else "inputs fit L2: not a bench workload",

@@ -45,8 +45,8 @@ const char* check_config(const sim_config* c) {
   if (!c) return "cfg is NULL";
   if (c->struct_size != sizeof(sim_config)) return "cfg.struct_size != sizeof(sim_config) (ABI mismatch)";
   if (c->n_gates < 1 || c->n_gates > 1024) return "n_gates must be in 1..1024";
-  if (c->n_doppler < 16 || c->n_doppler > 1024 || (c->n_doppler & (c->n_doppler - 1)))
-    return "n_doppler must be a power of two in 16..1024";
+  if (c->n_doppler < 16 || c->n_doppler > 2048 || (c->n_doppler & (c->n_doppler - 1)))
+    return "n_doppler must be a power of two in 16..2048";
   if (c->pulses_per_update < 1) return "pulses_per_update must be >= 1";
   if (c->max_pending_updates < 2) return "max_pending_updates must be >= 2";
   if (c->weight_mode != SIM_W_SQRT && c->weight_mode != SIM_W_LINEAR) return "unknown weight_mode";
@@ -744,7 +744,7 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       return SIM_OK;
     case SIM_OPT_ACC_WINDOW_BINS:
       if (h->opt_variant != 3 && (value & (value - 1))) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two (any width with variant 3)");
-      if (value > 1024) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 1024");
+      if (value > 2048) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 2048");
       h->opt_window = (int)value;
       if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
       if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");

@@ -143,6 +143,7 @@ static SynKernel syn_kernel(int logN) {
     case 8: return synth_kernel<8>;
     case 9: return synth_kernel<9>;
     case 10: return synth_kernel<10>;
+    case 11: return synth_kernel<11>;
     default: return nullptr;
   }
 }

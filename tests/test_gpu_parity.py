@@ -479,8 +479,31 @@ def test_regular_mode_errors(sim_mod):
     assert sim.regular_pulses(scat, sim_mod.sat_for(wl, 0), 0, 0).numel() == 0
 
 
+# ---- the paper's own sizes (n_fast = 250 ... 1250; PAPER.md:73 fence-post) ----
+@pytest.mark.parametrize("P,N", [(250, 256), (500, 512), (1000, 1024), (1250, 2048)])
+def test_paper_shaped_update_intervals(oracle, sim_mod, P, N):
+    """n_fast is not a power of two in the paper: the Doppler axis takes the next power of two (the long signal of
+    an update then covers its two segments without wrapping onto itself), and the track is synthesised the paper's
+    way: 1 + n_pulses / n_fast spectra, every segment bracketed by two of them (no tail rule)."""
+    wl = W.get("nadir_patch_16m").scaled(n_along=200, n_cross=256, n_doppler=N, pulses_per_update=P, n_updates=4)
+    scat = W.scatterers(wl)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    sim = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=wl.n_updates))
+    for u in range(wl.n_updates):
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
+        assert U.rel_l2(sim.get_spectrum(u).cpu().numpy(), T_ref[u]) <= U.TOL
+    n = (wl.n_updates - 1) * P                                   # whole-track batch post-processing, no SYN_FINAL
+    iq = sim.synthesize_pulses(n).cpu().numpy()
+    Y = oracle.synthesize(U.oracle_cfg(oracle, wl), T_ref, 0, n, final=False)
+    for s in range(wl.n_updates - 1):
+        assert U.rel_l2(iq[s * P:(s + 1) * P], Y[s * P:(s + 1) * P]) <= U.TOL
+    with pytest.raises(sim_mod.SimError):
+        sim.synthesize_pulses(1)                                  # the next segment has no successor yet
+
+
 def test_maximum_sizes(oracle, sim_mod):
-    wl = W.get("tiny").scaled(n_along=256, n_cross=256, n_gates=1024, n_doppler=1024, pulses_per_update=1024,
+    wl = W.get("tiny").scaled(n_along=256, n_cross=256, n_gates=1024, n_doppler=2048, pulses_per_update=2048,
                               n_updates=2, gate_spacing_m=0.05)
     scat = W.scatterers(wl)
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
@@ -535,7 +558,7 @@ def test_argument_errors(sim_mod):
     with pytest.raises(sim_mod.SimError):
         sim.accumulate_update(scat, sim_mod.make_sat((0, 0, 1), (0, 0, 0), (0, 0, 0), 0.0))   # zero boresight
     with pytest.raises(sim_mod.SimError):
-        sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, 2048)       # wider than the largest N
+        sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, 4096)       # wider than the largest N
     with pytest.raises(sim_mod.SimError):
         sim.set_option(sim_mod.OPT_ACC_EPOCH, 1 << 20)          # beyond the overflow-safe epoch length
     sim.set_option(sim_mod.OPT_ACC_VARIANT, 2)
