@@ -22,8 +22,8 @@ namespace simk {
 
 constexpr int kW3MaxStages = 6;
 
-// epoch parameter slot (ring of 4): 8 ints
-enum { kS3State = 0, kS3K0 = 1, kS3Ex = 2, kS3Gmin = 3, kS3Gmax = 4, kS3Ints = 8 };
+// epoch parameter slot (ring of 4): state, first bin of the Doppler window, scale exponent
+enum { kS3State = 0, kS3K0 = 1, kS3Ex = 2, kS3Ints = 4 };
 enum { kT3Unset = 0, kT3Claimed = 1, kT3Ready = 2 };
 
 int acc_ws3_chunk(int ncw, int pt) { return ncw * 32 * pt; }
@@ -124,11 +124,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
   const unsigned last_a = sh::addr(&s_last);
 
   for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * (NCW + 2) * 32) sh::st(tile0 + a, 0);
-  if (tid < 4) {
-    sh::st(slot0 + 4u * kS3Ints * tid + 4 * kS3State, kT3Unset);
-    sh::st(slot0 + 4u * kS3Ints * tid + 4 * kS3Gmin, INT_MAX);
-    sh::st(slot0 + 4u * kS3Ints * tid + 4 * kS3Gmax, INT_MIN);
-  }
+  if (tid < 4) sh::st(slot0 + 4u * kS3Ints * tid + 4 * kS3State, kT3Unset);
   if (tid == 0) {
     sh::st(last_a, (int)kFull);
     for (int s = 0; s < S; ++s) {
@@ -168,8 +164,8 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
       if (sh::ld(slot + 4 * kS3State) == kT3Ready) {
         const int k0 = sh::ld(slot + 4 * kS3K0), ex = sh::ld(slot + 4 * kS3Ex);
         const float inv_s = __int_as_float((127 - ex) << 23);
-        const int r0 = max(sh::ld(slot + 4 * kS3Gmin), 0), r1 = min(sh::ld(slot + 4 * kS3Gmax) + 1, G - 1);
-        const int ncell = (r1 >= r0) ? (r1 - r0 + 1) << logW : 0;   // nothing fitted (all escaped): empty range
+        const int r0 = 0, r1 = G - 1;   // every row: tracking the touched rows costs the compute warps more than the scan costs here
+        const int ncell = (r1 - r0 + 1) << logW;
         const unsigned tile = tile0 + b * tile_bytes;
         // four cells per lane per pass, their eight loads in flight together: the drain must be well under one
         // epoch long or the compute warps wait for their tile (profiles/r01_v3_final.md)
@@ -197,11 +193,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
           }
         }
         __syncwarp();
-        if (lane == 0) {
-          sh::st(slot + 4 * kS3State, kT3Unset);
-          sh::st(slot + 4 * kS3Gmin, INT_MAX);
-          sh::st(slot + 4 * kS3Gmax, INT_MIN);
-        }
+        if (lane == 0) sh::st(slot + 4 * kS3State, kT3Unset);
       }
       __syncwarp();
       if (lane == 0) sh::mbar_arrive(tfree0 + 8u * b);  // release: zeroed tile and reset slot are visible
@@ -224,7 +216,6 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
     bool have = false;         // this warp holds the epoch's parameters
     int k0 = 0, lo_bits = 0;
     float s = 0.0f;
-    int gmin = INT_MAX, gmax = INT_MIN;
     int ci = 0;
     for (; ci < EC; ++ci) {
       wait3(full0 + 8u * stg, ph, p.wait_hint);
@@ -379,8 +370,6 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
             sh::red_add(a0 + 4u * (unsigned)RS, fx_round3(c[j].x, w1s));
             sh::red_add(a0 + 4u * (unsigned)RS + plane_bytes, fx_round3(c[j].y, w1s));
           }
-          gmin = min(gmin, fits ? ix[j].g0 : INT_MAX);
-          gmax = max(gmax, fits ? ix[j].g0 : INT_MIN);
           esc[j] = ok[j] && !fits;
           esc_any |= esc[j];
         }
@@ -399,17 +388,9 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
       }
     }
 
-    // ---- end of an epoch (or of the input inside one): row range of what this warp added, tile to the drain warp ----
+    // ---- end of an epoch (or of the input inside one): tile to the drain warp ----
     {
       if (!more && lane == 0) sh::st(last_a, (int)e);   // the final epoch (possibly empty): the drain warp stops after it
-      if (have) {
-        gmin = __reduce_min_sync(kFull, gmin);
-        gmax = __reduce_max_sync(kFull, gmax);
-        if (lane == 0 && gmin <= gmax) {
-          sh::red_min(slot + 4 * kS3Gmin, gmin);
-          sh::red_max(slot + 4 * kS3Gmax, gmax);
-        }
-      }
       __syncwarp();
       if (lane == 0) sh::mbar_arrive(tdone0 + 8u * (e & 1u));
     }
