@@ -29,7 +29,6 @@ namespace simk {
 
 constexpr int kWsPT = 2;          // scatterers per lane per chunk (one 8-byte shared load per array)
 constexpr int kWsMaxStages = 4;
-constexpr int kMaxEpochAdds = 2047;
 
 // epoch parameter slot (ring of 4): 8 ints
 enum { kSlState = 0, kSlK0 = 1, kSlEx = 2, kSlGmin = 3, kSlGmax = 4, kSlInts = 8 };
