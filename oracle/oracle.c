@@ -422,6 +422,38 @@ int oracle_regular(const oracle_config *c, const oracle_sat *s, int64_t n, const
 #endif
 }
 
+/* Delay-Doppler burst step: "splitting the data into bursts of 64 pulses,
+ * and for each burst performing ... an along-track FFT".  Forward DFT along the pulses of each burst, per gate,
+ * written out: Z[b][k][g] = sum_{m<B} Y[b B + m][g] exp(-2 pi i ((k m) mod B)/B), unnormalised, k in natural order.
+ * The Doppler-centroid and range-migration corrections of the paper need instrument data and are not part of it.
+ * Y: [n_bursts * B][G], Z: [n_bursts][B][G], complex128. */
+int oracle_burst_dft(int32_t G, int32_t B, int64_t n_bursts, const double *Y, double *Z) {
+  if (G < 1 || B < 1 || n_bursts < 0 || !Y || !Z) return -1;
+  double *w = (double *)malloc((size_t)B * 2 * sizeof(double));
+  if (!w) return -2;
+  for (int j = 0; j < B; ++j) {
+    w[2 * j] = cos(TWO_PI * (double)j / (double)B);
+    w[2 * j + 1] = -sin(TWO_PI * (double)j / (double)B);
+  }
+#pragma omp parallel for schedule(static)
+  for (int64_t b = 0; b < n_bursts; ++b)
+    for (int k = 0; k < B; ++k)
+      for (int g = 0; g < G; ++g) {
+        double sr = 0.0, si = 0.0;
+        for (int m = 0; m < B; ++m) {
+          const double *y = Y + (((size_t)b * B + m) * G + g) * 2;
+          const int j = (int)(((int64_t)k * m) % B);
+          sr += y[0] * w[2 * j] - y[1] * w[2 * j + 1];
+          si += y[0] * w[2 * j + 1] + y[1] * w[2 * j];
+        }
+        double *z = Z + (((size_t)b * B + k) * G + g) * 2;
+        z[0] = sr;
+        z[1] = si;
+      }
+  free(w);
+  return 0;
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

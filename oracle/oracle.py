@@ -78,6 +78,8 @@ def lib():
         L.oracle_regular.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
                                      fp, fp, fp, fp, fp, fp, fp, C.c_int64, C.c_int64, dp, C.c_int, C.c_int]
         L.oracle_regular.restype = C.c_int
+        L.oracle_burst_dft.argtypes = [C.c_int32, C.c_int32, C.c_int64, dp, dp]
+        L.oracle_burst_dft.restype = C.c_int
         L.oracle_idft.argtypes = [C.c_int32, C.c_int32, dp, dp]
         L.oracle_idft.restype = C.c_int
         L.oracle_weight.argtypes = [C.c_int32, C.c_int32, C.c_int64]
@@ -169,6 +171,19 @@ def regular(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz, s0dA, j0, n_
     if rc < 0:
         raise RuntimeError(f"oracle_regular failed: {rc}")
     return Y
+
+
+def burst_dft(Y, burst):
+    """Delay-Doppler burst step: forward DFT along the pulses of each burst.  Y [n_pulses][G] -> [n_bursts][burst][G]."""
+    Y = np.ascontiguousarray(Y, dtype=np.complex128)
+    n, G = Y.shape
+    assert n % burst == 0
+    Z = np.empty((n // burst, burst, G), dtype=np.complex128)
+    rc = lib().oracle_burst_dft(G, int(burst), n // burst, Y.ctypes.data_as(C.POINTER(C.c_double)),
+                                Z.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc < 0:
+        raise RuntimeError(f"oracle_burst_dft failed: {rc}")
+    return Z
 
 
 def idft(T):
