@@ -169,6 +169,14 @@ int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset)
 int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat,
                        int64_t first_pulse, int64_t n_pulses, void* d_iq, uint32_t flags);
 
+/* Delay-Doppler burst step (reading R8): the IQ stream is split into
+ * bursts of `burst` pulses (64 in the paper; a power of two in 16..128) and each burst gets an along-track FFT per
+ * gate: beams[b][k][g] = sum_m iq[b burst + m][g] exp(-2 pi i k m / burst), unnormalised, beam k in natural FFT order.
+ * d_iq: DEVICE complex64 [n_pulses][G]; d_beams: DEVICE complex64 [n_pulses / burst][burst][G]; out of place; 16-byte
+ * aligned; n_pulses a multiple of burst.  The Doppler-centroid and range-migration corrections of the paper need
+ * instrument data and are not part of it. */
+int sim_burst_beams(sim_handle* h, const void* d_iq, int64_t n_pulses, int32_t burst, void* d_beams, uint32_t flags);
+
 /* Runs the production index computation only: for each scatterer the gate g0 = floor(gf) in
  * [-1, G-1] and the Doppler bin k in [0, N); dropped scatterers give (SIM_GATE_NONE, -1).
  * d_gate0, d_bin: DEVICE int32[n].  Must match the canonical fp64 sequence bit for bit. */

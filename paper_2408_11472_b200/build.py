@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(CSRC, "libsim.so")
-SOURCES = ["sim_api.cu", "accumulate.cu", "accumulate_ws.cu", "accumulate_ws3.cu", "synthesize.cu", "regular.cu"]
+SOURCES = ["sim_api.cu", "accumulate.cu", "accumulate_ws.cu", "accumulate_ws3.cu", "synthesize.cu", "regular.cu", "burst.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
 

@@ -657,6 +657,25 @@ int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sa
   return SIM_OK;
 }
 
+int sim_burst_beams(sim_handle* h, const void* d_iq, int64_t n_pulses, int32_t burst, void* d_beams, uint32_t flags) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (flags) return fail(h, SIM_ERR_INVALID_ARG, "unknown burst flag");
+  if (burst < 16 || burst > 128 || (burst & (burst - 1))) return fail(h, SIM_ERR_INVALID_ARG, "burst must be a power of two in 16..128");
+  if (n_pulses < 0 || n_pulses % burst) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses must be a non-negative multiple of burst");
+  if (n_pulses == 0) return SIM_OK;
+  if (!d_iq || !d_beams) return fail(h, SIM_ERR_INVALID_ARG, "iq / beams buffer is NULL");
+  if (d_iq == d_beams) return fail(h, SIM_ERR_INVALID_ARG, "the transform is out of place: iq and beams must differ");
+  if (misaligned(d_iq) || misaligned(d_beams)) return fail(h, SIM_ERR_INVALID_ARG, "iq / beams buffers must be 16-byte aligned");
+  int logB = 0;
+  while ((1 << logB) < burst) ++logB;
+  int l = 0;
+  const cudaError_t e = launch_burst_fft(static_cast<const float2*>(d_iq), static_cast<float2*>(d_beams), n_pulses / burst, logB,
+                                         h->cfg.n_gates, h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) return cuda_fail(h, e, "burst FFT launch");
+  return SIM_OK;
+}
+
 int sim_synchronize(sim_handle* h) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   cudaError_t e = cudaStreamSynchronize(h->stream);

@@ -113,6 +113,9 @@ cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks,
 // large for one pulse row per thread in shared memory
 cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,
                            size_t smem_optin, cudaStream_t st, int* launches);
+// Delay-Doppler burst step (burst.cu): Z[b][k][g] = forward FFT over the 2^logB pulses of burst b, per gate
+cudaError_t launch_burst_fft(const float2* Y, float2* Z, long long n_bursts, int logB, int G, cudaStream_t st,
+                             int* launches);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
 int synth_gate_tile(int N, int G, long long n_segments, int sm_count);

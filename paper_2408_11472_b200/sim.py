@@ -28,7 +28,7 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",
     "sim_accumulate_update_host", "sim_synthesize_pulses_host", "sim_synchronize", "sim_destroy",
     "sim_get_spectrum", "sim_spectrum_offset", "sim_debug_indices", "sim_set_option", "sim_get_stats",
-    "sim_read_counters", "sim_last_error", "sim_regular_pulses",
+    "sim_read_counters", "sim_last_error", "sim_regular_pulses", "sim_burst_beams",
 ]
 
 
@@ -197,6 +197,17 @@ class Sim:
         self._check(self.lib.sim_regular_pulses(self._h, C.byref(s), C.byref(sat), C.c_int64(first_pulse),
                                                 C.c_int64(n_pulses), C.c_void_p(out.data_ptr()), C.c_uint32(flags)),
                     self._h)
+        return out
+
+    def burst_beams(self, iq: torch.Tensor, burst: int = 64):
+        """Delay-Doppler burst step (sim_burst_beams): [n_pulses][G] -> [n_pulses / burst][burst][G] complex64."""
+        G = self.cfg.n_gates
+        if iq.dtype != torch.complex64 or not iq.is_contiguous() or not iq.is_cuda or iq.shape[-1] != G:
+            raise ValueError("iq must be a contiguous CUDA complex64 tensor [n_pulses][G]")
+        n = iq.shape[0]
+        out = torch.empty((n // max(burst, 1), burst, G), dtype=torch.complex64, device=self.device)
+        self._check(self.lib.sim_burst_beams(self._h, C.c_void_p(iq.data_ptr()), C.c_int64(n), C.c_int32(burst),
+                                             C.c_void_p(out.data_ptr()), C.c_uint32(0)), self._h)
         return out
 
     def accumulate_update_host(self, scat: dict, sat: SimSatState, flags: int = 0):

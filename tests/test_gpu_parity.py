@@ -502,6 +502,23 @@ def test_paper_shaped_update_intervals(oracle, sim_mod, P, N):
         sim.synthesize_pulses(1)                                  # the next segment has no successor yet
 
 
+# ---- Delay-Doppler burst step -------------------------------------
+@pytest.mark.parametrize("burst", [16, 64, 128])
+def test_burst_beams(oracle, sim_mod, burst):
+    wl = W.get("tiny").scaled(n_along=96, n_cross=96, n_gates=70, n_updates=5, n_doppler=128, pulses_per_update=128)
+    scat_cuda = U.to_cuda(W.scatterers(wl))
+    _, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda)                 # 640 pulses x 70 gates (a ragged gate tile)
+    Z = sim.burst_beams(torch.from_numpy(iq).cuda(), burst).cpu().numpy()
+    Z_ref = oracle.burst_dft(iq, burst)
+    assert Z.shape == Z_ref.shape == (640 // burst, burst, 70)
+    for b in range(Z.shape[0]):
+        assert U.rel_l2(Z[b], Z_ref[b]) <= U.TOL
+    with pytest.raises(sim_mod.SimError):
+        sim.burst_beams(torch.from_numpy(iq[:100]).cuda(), 64)     # not a multiple of the burst
+    with pytest.raises(sim_mod.SimError):
+        sim.burst_beams(torch.from_numpy(iq).cuda(), 48)           # not a power of two
+
+
 def test_maximum_sizes(oracle, sim_mod):
     wl = W.get("tiny").scaled(n_along=256, n_cross=256, n_gates=1024, n_doppler=2048, pulses_per_update=2048,
                               n_updates=2, gate_spacing_m=0.05)
