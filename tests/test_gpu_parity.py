@@ -115,6 +115,22 @@ def test_full_sar_footprint_268m(oracle, sim_mod):
     assert 0.5 < frac < 0.65, frac          # pi * 6985^2 / 16384^2 = 0.57 (DESIGN.md input recipe)
 
 
+def test_full_track_segment_67m(oracle, sim_mod):
+    """configs[4] at full size (67M scatterers, 16384 along x 4096 cross): the first and the last of the 64 updates
+    (the satellite 3.2 km before and after the strip's centre; a few scatterers alias in Doppler at the far end)."""
+    wl = W.get("track_segment_67m")
+    scat_cuda = W.scatterers(wl, device="cuda")
+    scat_np = U.to_numpy(scat_cuda)
+    sim = sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=2))
+    for j, u in enumerate((0, wl.n_updates - 1)):
+        T_ref = U.oracle_spectra(oracle, wl, scat_np, [u])[0]
+        sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
+        e = U.rel_l2(sim.get_spectrum(j).cpu().numpy(), T_ref)
+        assert e <= U.TOL, f"update {u}: {e}"
+        n_in = _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=u)
+        assert 0.5 < n_in / wl.n_scatterers <= 1.0
+
+
 # ---- stream semantics --------------------------------------------------------------------------------
 @pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("N,P", [(64, 64), (64, 48), (32, 100), (128, 64)])
