@@ -203,7 +203,8 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_EPOCH 12     /* scatterers per fixed-point epoch: variant 2 64..2047 (default 2047), variant 3 64..16383 (default 8191) */
 #define SIM_OPT_ACC_WAIT_HINT 13 /* variant 3: suspend-time hint (ns) of the compute warps' mbarrier waits; 0 (default) =
                                     plain try_wait loop (the control warps always sleep) */
-#define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 = scheduling units visit the scene in a scattered order, 0 (default) = in order */
+#define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 (default) = scheduling units visit the scene in a scattered order (dark and
+                                    illuminated parts in flight together), 0 = in order */
 #define SIM_OPT_ACC_INTERLEAVE 15 /* variant 3: scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
 #define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);

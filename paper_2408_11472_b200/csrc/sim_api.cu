@@ -506,7 +506,7 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   variant_defaults(h);
   h->opt_stages = 0;
   h->opt_wait_hint = 0;
-  h->opt_scatter = 0;
+  h->opt_scatter = 1;
   h->opt_blocks = 0;
   h->opt_window = 0;
   h->opt_index_path = 1;

@@ -358,7 +358,7 @@ def test_v3_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
     scat = W.scatterers(wl)
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
-    for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 1}), (4095, {sim_mod.OPT_ACC_STAGES: 2, sim_mod.OPT_ACC_WINDOW_BINS: 11}),
+    for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 0}), (4095, {sim_mod.OPT_ACC_STAGES: 2, sim_mod.OPT_ACC_WINDOW_BINS: 11}),
                          (8191, {sim_mod.OPT_ACC_SUPERCHUNK: 1}), (16383, {sim_mod.OPT_ACC_BLOCKS: 3})):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
         sim.set_option(sim_mod.OPT_ACC_VARIANT, 3)
