@@ -164,7 +164,7 @@ int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset)
  * gates (the linear split of step A3).  d_iq: DEVICE complex64 [n_pulses][G], gate fastest, 16-byte aligned.
  * flags = 0: d_iq is zeroed first; SIM_ACC_APPEND: the sums are added to it (scenes delivered in pieces).
  * Work is scatterers x pulses.  Independent of the spectra ring and of sim_synthesize_pulses.
- * Errors: SIM_ERR_INVALID_ARG (NULL / misaligned), SIM_ERR_BAD_CONFIG (n_gates > ~768, or a gate window too
+ * Errors: SIM_ERR_INVALID_ARG (NULL / misaligned), SIM_ERR_BAD_CONFIG (n_gates > ~830, or a gate window too
  * deep for the polynomial gate coordinate). */
 int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat,
                        int64_t first_pulse, int64_t n_pulses, void* d_iq, uint32_t flags);

@@ -4,81 +4,79 @@
 //     Y[j][g] = sum_p w_g(R_p(t_j)) sqrt(s0dA_p) G(theta_p(t_j)) / R_p(t_j)^2 exp(-i 4 pi R_p(t_j) / lambda),  t_j = j / PRF.
 // Work = scatterers x pulses.  No Doppler axis, no FFT: this is the at-scale truth the fast mode approximates.
 //
-// One THREAD = one PULSE with a private row Y[j][0..G) in shared memory (plain read-modify-write, no atomics);
-// a block = JT pulses x one slice of the scatterers.  The block's threads first turn a chunk of scatterers into
-// per-scatterer constants (u(t) = R(t)^2 - rg0^2 = u0 + a t + b t^2 in fp64, antenna projections linear in t),
-// then every thread walks the chunk (shared-memory broadcasts).  Per (scatterer, pulse): 2 DFMA for u, the gate
-// coordinate by the same polynomial as the fast-mode index path, phase fraction in fp64, the rest in fp32.
-// At the end the block adds its tile to Y with red.global.add.v2.f32.
+// One WARP = one SCATTERER at a time, its 32 LANES = the 32 PULSES of the block's pulse tile; a block = 16 warps x one
+// slice of the scatterers, with a shared-memory tile Y[32 pulses][G] in fp32.  Lanes of a warp always hit different
+// rows (pulses), so the shared-memory adds of a warp never collide with each other; warps collide only when two
+// scatterers fall into the same gate at the same pulse at the same moment, which fp32 atomicAdd (a CAS loop on
+// sm_100a) resolves with few retries.  The block's threads first turn a chunk of scatterers into per-scatterer
+// constants (u(t) = R(t)^2 - rg0^2 = u0 + a t + b t^2 in fp64, antenna projections linear in t; raw inputs of the
+// next chunk prefetched into registers), then every warp walks its share of the chunk (shared-memory broadcasts).
+// Per (scatterer, pulse): 2 DFMA for u, the gate coordinate by the same polynomial as the fast-mode index path,
+// phase fraction in fp64, the rest in fp32.  At the end the block adds its tile to Y with red.global.add.v2.f32.
 #include "scatter_math.cuh"
 
 namespace simk {
 
-constexpr int kRegChunk = 256;   // scatterers per shared-memory chunk
+constexpr int kRegWarps = 16;                  // warps per block
+constexpr int kRegThreads = kRegWarps * 32;
+constexpr int kRegChunk = kRegThreads;         // scatterers per shared-memory chunk: one per thread to prepare
+constexpr int kRegJT = 32;                     // pulses per block = lanes of a warp
 
 struct RegParams {
   AccParams a;       // geometry constants (make_acc_params)
   float2* Y;         // [n_pulses][G]
   long long j0;      // first pulse, relative to the instant of the satellite state
-  int n_pulses, JT;  // pulses of the call, pulses (= threads) per block
+  int n_pulses;      // pulses of the call
   int n_slices;      // scatterer slices (gridDim.y)
   double prf;        // t_j = j / PRF, the oracle's expression
 };
 
-size_t regular_smem_bytes(int G, int JT) {
-  return (size_t)JT * (2 * G + 1) * sizeof(float) + (size_t)kRegChunk * (3 * sizeof(double) + 6 * sizeof(float));
+size_t regular_smem_bytes(int G) {
+  return (size_t)kRegJT * (2 * G + 1) * sizeof(float) + (size_t)kRegChunk * (3 * sizeof(double) + 6 * sizeof(float));
 }
 
-__global__ void regular_kernel(RegParams rp) {
+__global__ void __launch_bounds__(kRegThreads) regular_kernel(RegParams rp) {
   const AccParams& p = rp.a;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int G = p.G, JT = rp.JT, LD = 2 * G + 1;
+  const int G = p.G, LD = 2 * G + 1;
   double* s_u0 = reinterpret_cast<double*>(smem_raw);   // [chunk] u at pulse 0
   double* s_a = s_u0 + kRegChunk;                        // [chunk] 2 d.dv
   double* s_b = s_a + kRegChunk;                         // [chunk] |dv|^2
-  float* s_p1 = reinterpret_cast<float*>(s_b + kRegChunk);   // [chunk] d.e1, then dv.e1, d.e2, dv.e2, sqrt(s0dA), live
+  float* s_p1 = reinterpret_cast<float*>(s_b + kRegChunk);   // [chunk] d.e1, then dv.e1, d.e2, dv.e2, sqrt(s0dA)
   float* s_p1v = s_p1 + kRegChunk;
   float* s_p2 = s_p1v + kRegChunk;
   float* s_p2v = s_p2 + kRegChunk;
   float* s_amp = s_p2v + kRegChunk;
   float* s_pad = s_amp + kRegChunk;                      // (unused sixth array keeps the tile 8-byte aligned)
-  float* tile = s_pad + kRegChunk;                       // [JT][2G+1]: re, im interleaved per gate
-  const int tid = threadIdx.x;
-  float* row = tile + (size_t)tid * LD;
-  for (int i = 0; i < LD; ++i) row[i] = 0.0f;
+  float* tile = s_pad + kRegChunk;                       // [32 pulses][2G+1]: re, im interleaved per gate
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int i = tid; i < kRegJT * LD; i += kRegThreads) tile[i] = 0.0f;
+  float* row = tile + (size_t)lane * LD;
 
-  const long long j = rp.j0 + (long long)blockIdx.x * JT + tid;
-  const bool pulse_ok = (long long)blockIdx.x * JT + tid < rp.n_pulses;
+  const long long j = rp.j0 + (long long)blockIdx.x * kRegJT + lane;
+  const bool pulse_ok = (long long)blockIdx.x * kRegJT + lane < rp.n_pulses;
   const double t = __ddiv_rn((double)j, rp.prf);
   const float tf = (float)t;
 
   const unsigned long long per = (p.n + rp.n_slices - 1) / rp.n_slices;
   const unsigned long long lo = per * blockIdx.y, hi = (lo + per < p.n) ? lo + per : p.n;
-  // Each thread prepares up to kPrep scatterers of a chunk.  Their raw inputs are fetched into registers one chunk
-  // ahead, so that the global-load latency is hidden behind the evaluation of the current chunk.
-  constexpr int kPrep = (kRegChunk + 31) / 32;   // enough for the smallest block (32 threads)
-  float in[kPrep][7];
-  auto fetch = [&](unsigned long long base) {
-#pragma unroll
-    for (int k = 0; k < kPrep; ++k) {
-      const unsigned long long q = base + tid + (unsigned long long)k * JT;
-      const bool v = tid + k * JT < kRegChunk && q < hi;
-      in[k][0] = v ? p.x[q] : 0.0f; in[k][1] = v ? p.y[q] : 0.0f; in[k][2] = v ? p.z[q] : 0.0f;
-      in[k][3] = v ? p.vx[q] : 0.0f; in[k][4] = v ? p.vy[q] : 0.0f; in[k][5] = v ? p.vz[q] : 0.0f;
-      in[k][6] = v ? p.s0dA[q] : 0.0f;
-    }
+  float in[7];
+  auto fetch = [&](unsigned long long base) {   // this thread's scatterer of the chunk at `base`, raw
+    const unsigned long long q = base + tid;
+    const bool v = q < hi;
+    in[0] = v ? p.x[q] : 0.0f; in[1] = v ? p.y[q] : 0.0f; in[2] = v ? p.z[q] : 0.0f;
+    in[3] = v ? p.vx[q] : 0.0f; in[4] = v ? p.vy[q] : 0.0f; in[5] = v ? p.vz[q] : 0.0f;
+    in[6] = v ? p.s0dA[q] : 0.0f;
   };
   if (lo < hi) fetch(lo);
   for (unsigned long long base = lo; base < hi; base += kRegChunk) {
     const int m = (int)((hi - base < (unsigned long long)kRegChunk) ? hi - base : kRegChunk);
-    __syncthreads();   // the previous chunk has been consumed
-#pragma unroll
-    for (int k = 0; k < kPrep; ++k) {
-      const int i = tid + k * JT;
-      if (i >= m) continue;
-      const float s0 = in[k][6];
-      const double dx = __dsub_rn((double)in[k][0], p.sx), dy = __dsub_rn((double)in[k][1], p.sy), dz = __dsub_rn((double)in[k][2], p.sz);
-      const double dvx = (double)in[k][3] - p.svx, dvy = (double)in[k][4] - p.svy, dvz = (double)in[k][5] - p.svz;
+    __syncthreads();   // the previous chunk has been consumed (and, the first time, the tile is zero)
+    if (tid < m) {
+      const int i = tid;
+      const float s0 = in[6];
+      const double dx = __dsub_rn((double)in[0], p.sx), dy = __dsub_rn((double)in[1], p.sy), dz = __dsub_rn((double)in[2], p.sz);
+      const double dvx = (double)in[3] - p.svx, dvy = (double)in[4] - p.svy, dvz = (double)in[5] - p.svz;
       s_u0[i] = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.neg_rg0sq)));
       s_a[i] = 2.0 * fma(dvz, dz, fma(dvy, dy, dvx * dx));
       s_b[i] = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
@@ -92,10 +90,11 @@ __global__ void regular_kernel(RegParams rp) {
     if (base + kRegChunk < hi) fetch(base + kRegChunk);   // in flight during the evaluation below
     if (!pulse_ok) continue;
 #pragma unroll 2
-    for (int i = 0; i < m; ++i) {
+    for (int i = warp; i < m; i += kRegWarps) {   // warp-uniform: every lane reads the same scatterer (broadcast)
       const float amp = s_amp[i];
+      if (!(amp > 0.0f)) continue;
       const double u = fma(t, fma(t, s_b[i], s_a[i]), s_u0[i]);
-      if (!(amp > 0.0f) || !(u >= p.uw_lo && u <= p.uw_hi)) continue;   // dead, or outside the window (NaN too)
+      if (!(u >= p.uw_lo && u <= p.uw_hi)) continue;              // outside the window at this pulse (NaN too)
       const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
       const int gfx = __double2loint(__dadd_rd(gf, kMagicFx));   // floor(gf * 2^20)
       const int g0 = gfx >> kFracBits;
@@ -110,32 +109,30 @@ __global__ void regular_kernel(RegParams rp) {
       __sincosf(6.283185307179586f * fr, &sn, &cs);
       const float re = A * cs, im = -A * sn, w0 = 1.0f - w1;
       if (g0 >= 0) {
-        row[2 * g0] = fmaf(w0, re, row[2 * g0]);
-        row[2 * g0 + 1] = fmaf(w0, im, row[2 * g0 + 1]);
+        atomicAdd(&row[2 * g0], w0 * re);
+        atomicAdd(&row[2 * g0 + 1], w0 * im);
       }
       if (g0 + 1 < G) {
-        row[2 * g0 + 2] = fmaf(w1, re, row[2 * g0 + 2]);
-        row[2 * g0 + 3] = fmaf(w1, im, row[2 * g0 + 3]);
+        atomicAdd(&row[2 * g0 + 2], w1 * re);
+        atomicAdd(&row[2 * g0 + 3], w1 * im);
       }
     }
   }
   __syncthreads();
   // ---- flush: gate fastest across threads so that the reductions of a warp hit consecutive addresses ----
-  const int rows = min(JT, rp.n_pulses - blockIdx.x * JT);
-  for (int e = tid; e < rows * G; e += JT) {
+  const int rows = min(kRegJT, rp.n_pulses - blockIdx.x * kRegJT);
+  for (int e = tid; e < rows * G; e += kRegThreads) {
     const int r = e / G, g = e - r * G;
     const float re = tile[(size_t)r * LD + 2 * g], im = tile[(size_t)r * LD + 2 * g + 1];
-    if (re != 0.0f || im != 0.0f) atomicAdd(&rp.Y[((size_t)blockIdx.x * JT + r) * G + g], make_float2(re, im));
+    if (re != 0.0f || im != 0.0f) atomicAdd(&rp.Y[((size_t)blockIdx.x * kRegJT + r) * G + g], make_float2(re, im));
   }
 }
 
 cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,
                            size_t smem_optin, cudaStream_t st, int* launches) {
   if (n_pulses <= 0 || a.n == 0) return cudaSuccess;
-  int JT = 192;
-  while (JT > 32 && (JT - 32 >= n_pulses || regular_smem_bytes(a.G, JT) > smem_optin - 2048)) JT -= 32;
-  if (regular_smem_bytes(a.G, JT) > smem_optin - 2048) return cudaErrorInvalidConfiguration;
-  const size_t smem = regular_smem_bytes(a.G, JT);
+  const size_t smem = regular_smem_bytes(a.G);
+  if (smem > smem_optin - 2048) return cudaErrorInvalidConfiguration;
   cudaError_t e = cudaFuncSetAttribute(regular_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   RegParams rp;
@@ -143,15 +140,15 @@ cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pu
   rp.Y = Y;
   rp.j0 = j0;
   rp.n_pulses = n_pulses;
-  rp.JT = JT;
   rp.prf = prf;
-  const int tiles = (n_pulses + JT - 1) / JT;
-  int slices = (2 * sm_count + tiles - 1) / tiles;
+  const int tiles = (n_pulses + kRegJT - 1) / kRegJT;
+  int slices = (4 * sm_count + tiles - 1) / tiles;   // about four blocks per SM in total
   const unsigned long long max_slices = (a.n + kRegChunk - 1) / kRegChunk;
   if ((unsigned long long)slices > max_slices) slices = (int)max_slices;
   if (slices > 65535) slices = 65535;
+  if (slices < 1) slices = 1;
   rp.n_slices = slices;
-  regular_kernel<<<dim3(tiles, slices), JT, smem, st>>>(rp);
+  regular_kernel<<<dim3(tiles, slices), kRegThreads, smem, st>>>(rp);
   ++*launches;
   return cudaGetLastError();
 }
