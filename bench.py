@@ -339,7 +339,9 @@ def main():
         lo = (wl.n_along - rows) // 2 * wl.n_cross
         sub = {k: v[lo:lo + rows * wl.n_cross].cpu() for k, v in scat.items()}
         v, desc, used, _ = cpu_oracle_sample(wl, sub, orc.max_threads(), target_s=12.0)
-        cpu_baseline = {"value": v, "unit": "scatterers/s", "cores": used, "kind": "oracle", "sample": desc}
+        v1, _, _, _ = cpu_oracle_sample(wl, sub, 1, target_s=3.0)     # the same oracle on one core (BASELINE.md plan)
+        cpu_baseline = {"value": v, "unit": "scatterers/s", "cores": used, "kind": "oracle", "sample": desc,
+                        "single_thread_value": v1}
 
     if rank == 0:
         out = {
