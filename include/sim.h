@@ -196,7 +196,7 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_PER_THREAD 7 /* scatterers per thread per chunk of the tile kernel: 2 or 4 */
 #define SIM_OPT_ACC_MIN_BLOCKS 8 /* register budget of the tile kernel: compiled for 2..4 resident blocks per SM */
 #define SIM_OPT_ACC_WARPS 9      /* compute warps per block.  variant 2: 7, 14 (default), 22 or 30;
-                                    variant 3 (with per-lane, interleave): (8,4,2) default, (8,2,2), (8,4,4),
+                                    variant 3 (with per-lane, interleave): (8,4,4) default, (8,2,2), (8,4,2),
                                     (12,2,2), (16,4,2), (20,4,2) */
 #define SIM_OPT_ACC_STAGES 10    /* depth of the TMA stage ring: 0 = as many as fit, else 2..4 (variant 3: 2..6) */
 #define SIM_OPT_ACC_PER_LANE 11  /* variant 3: scatterers per lane per chunk: 2 or 4 */

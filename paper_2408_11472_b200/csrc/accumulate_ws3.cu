@@ -296,7 +296,9 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
             for (int j = 0; j < IL; ++j) {
               if (near[j]) {
                 ++fallbacks;
-                ok[j] = canonical(p, q[j].dx, q[j].dy, q[j].dz, vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ix[j]);
+                // offsets recomputed here (three subtractions) rather than kept alive across the amplitude for this rare case
+                ok[j] = canonical(p, __dsub_rn((double)x.v[gi + j], p.sx), __dsub_rn((double)y.v[gi + j], p.sy),
+                                  __dsub_rn((double)z.v[gi + j], p.sz), vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], ix[j]);
                 float A;
                 c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ix[j].gfx, ix[j].fr, s0.v[gi + j], A);
                 ab[j] = __float_as_int(A);
@@ -475,10 +477,19 @@ cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int sta
 
 cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, int blocks, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  W3Kernel k = ws3_kernel(ncw, pt, il, acc_index_mode(p));
+  const int mode = acc_index_mode(p);
+  // the canonical-everywhere path calls the out-of-line sequence once per scatterer: two in flight per lane are enough
+  const bool swapped = mode == kIdxCanonical && il == 4 && ws3_kernel(ncw, pt, 2, mode);
+  if (swapped) il = 2;
+  W3Kernel k = ws3_kernel(ncw, pt, il, mode);
   if (!k) return cudaErrorInvalidValue;
   const size_t smem = acc_ws3_smem_bytes(p.G, p.W, ncw, pt, p.stages);
-  cudaError_t e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
+  cudaError_t e = cudaSuccess;
+  if (swapped) {   // the plan set the shared-memory limit of the planned shape only
+    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+  }
+  e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
   if (e != cudaSuccess) return e;
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
   const int grid = (int)(n_sc < (unsigned long long)blocks ? n_sc : (unsigned long long)blocks);

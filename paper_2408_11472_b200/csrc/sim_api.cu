@@ -244,7 +244,7 @@ cudaError_t plan_tile(sim_handle* h) {
 // Per-variant defaults of the warp-specialised kernels (measured on the 268M config, profiles/).
 void variant_defaults(sim_handle* h) {
   if (h->opt_variant == 3) {
-    h->opt_ncw = 8; h->opt_pt = 4; h->opt_il = 2; h->opt_epoch = 8191;
+    h->opt_ncw = 8; h->opt_pt = 4; h->opt_il = 4; h->opt_epoch = 8191;
   } else {
     h->opt_ncw = 14; h->opt_pt = 2; h->opt_il = 2; h->opt_epoch = 2047;
   }

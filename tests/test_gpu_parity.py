@@ -362,7 +362,8 @@ def test_v3_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
                          (8191, {sim_mod.OPT_ACC_SUPERCHUNK: 1}), (16383, {sim_mod.OPT_ACC_BLOCKS: 3})):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
         sim.set_option(sim_mod.OPT_ACC_VARIANT, 3)
-        sim.set_option(sim_mod.OPT_ACC_PER_LANE, pt)        # each intermediate combination is a compiled shape
+        sim.set_option(sim_mod.OPT_ACC_INTERLEAVE, 2)       # each intermediate combination is a compiled shape
+        sim.set_option(sim_mod.OPT_ACC_PER_LANE, pt)
         sim.set_option(sim_mod.OPT_ACC_WARPS, ncw)
         sim.set_option(sim_mod.OPT_ACC_INTERLEAVE, il)
         sim.set_option(sim_mod.OPT_ACC_EPOCH, epoch)
