@@ -11,8 +11,16 @@
 //   * the two control warps wait with a suspend-time hint (v2 spent 20 % of its issue slots spinning); the block's
 //     end is signalled through the barriers themselves (the compute warps publish the index of the final epoch);
 //   * the tile has one padding row below gate 0 and one above gate G-1, so the two gate halves need no
-//     per-half bounds predicate;
-//   * fewer compute warps with more registers each (no spills), loop state kept in registers.
+//     per-half bounds predicate; the drain warp scans every row (tracking the touched rows cost the compute warps
+//     more than the scan costs the drain warp);
+//   * 8 compute warps with 96 registers each, 4 scatterers per lane per chunk, all four in flight together;
+//   * the polynomial index path runs straight through for the scatterers in flight and ONE cold block per group
+//     re-decides the rare guard-band cases: a call site in the hot flow cuts the live ranges of ~40 constants;
+//   * long fixed-point epochs (8191 scatterers by default) with an admitted magnitude range that shrinks as the
+//     epoch grows, so that no cell can overflow: every epoch boundary is a rendez-vous of the block's warps;
+//   * scheduling units are visited in a scattered order (golden-ratio stride), so that dark parts of the scene
+//     (DRAM-bound) and illuminated parts (issue-bound) are in flight at the same time.
+// Measurements and the experiments behind each choice: profiles/r01_v3_ws3_kernel.md, profiles/r01_v3_final.md.
 #include <climits>
 
 #include "ptx_util.cuh"
