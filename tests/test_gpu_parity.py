@@ -486,6 +486,29 @@ def test_regular_mode(oracle, sim_mod, name):
     assert U.rel_l2(T.sum(axis=1), Y0) <= U.TOL
 
 
+def test_regular_mode_heavy_tailed_amplitudes(oracle, sim_mod):
+    """The regular-mode tile is block floating point too: bright targets (x 1e6 in amplitude) leave the int32 range
+    and take the exact global reduction, a dim band and dead chunks keep the bound."""
+    wl = W.get("nadir_patch_16m").scaled(n_along=200, n_cross=512, n_updates=1)
+    scat = W.scatterers(wl)
+    g = torch.Generator().manual_seed(5)
+    s0 = scat["s0dA"]
+    s0[torch.randperm(s0.numel(), generator=g)[:200]] *= 1e12
+    s0[30_000:50_000] *= 1e-8
+    s0[60_000:60_512] = 0.0
+    s0[80_000:] *= torch.exp(4.0 * torch.randn(s0.numel() - 80_000, generator=g))
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    Y_ref = oracle.regular(U.oracle_cfg(oracle, wl), U.oracle_sat(oracle, wl, 0), *[scat_np[f] for f in W.FIELDS],
+                           -16, 80, nthreads=oracle.max_threads())
+    sim = sim_mod.Sim(sim_mod.config_for(wl))
+    Y = sim.regular_pulses(scat_cuda, sim_mod.sat_for(wl, 0), -16, 80).cpu().numpy()
+    assert U.rel_l2(Y, Y_ref) <= U.TOL
+    dim = {k: v[30_000:50_000].contiguous() for k, v in scat_cuda.items()}    # a scene that is dim everywhere
+    Yd_ref = oracle.regular(U.oracle_cfg(oracle, wl), U.oracle_sat(oracle, wl, 0),
+                            *[scat_np[f][30_000:50_000] for f in W.FIELDS], 0, 40, nthreads=oracle.max_threads())
+    assert U.rel_l2(sim.regular_pulses(dim, sim_mod.sat_for(wl, 0), 0, 40).cpu().numpy(), Yd_ref) <= U.TOL
+
+
 def test_regular_mode_errors(sim_mod):
     wl = W.get("tiny").scaled(n_gates=1024, gate_spacing_m=0.05)
     sim = sim_mod.Sim(sim_mod.config_for(wl))
