@@ -32,9 +32,9 @@ int synth_gate_tile(int N, int G, long long n_segments, int sm_count) {
   // two signals x GT rows x (N+1) float2 (+ the twiddle table) must fit comfortably in shared memory ...
   int gt = 16;
   while (gt > 1 && (size_t)2 * gt * (N + 1) * sizeof(float2) > 160 * 1024) gt >>= 1;
-  // ... and the grid should cover the machine twice: a call is a few segments x G gates, so small gate tiles
+  // ... and the grid should give every SM several blocks: a call is a few segments x G gates, so small gate tiles
   // are what gives it blocks.  Not below 2 gates (16-byte pieces of the gate-fastest IQ rows).
-  while (gt > 2 && n_segments * ((G + gt - 1) / gt) < 2LL * sm_count) gt >>= 1;
+  while (gt > 2 && n_segments * ((G + gt - 1) / gt) < 8LL * sm_count) gt >>= 1;
   return gt;
 }
 
