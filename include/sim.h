@@ -206,6 +206,7 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 (default) = scheduling units visit the scene in a scattered order (dark and
                                     illuminated parts in flight together), 0 = in order */
 #define SIM_OPT_ACC_INTERLEAVE 15 /* variant 3: scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
+#define SIM_OPT_ACC_SHAPE 16      /* block shape in one call: (warps << 16) | (per lane << 8) | interleave */
 #define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 

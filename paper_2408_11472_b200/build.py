@@ -1,38 +1,65 @@
-"""Builds csrc/libsim.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Builds csrc/libsim.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).  Every .cu is compiled to an
+object file under csrc/build/ (in parallel), then linked."""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
+OBJ = os.path.join(CSRC, "build")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(CSRC, "libsim.so")
-SOURCES = ["sim_api.cu", "accumulate.cu", "accumulate_ws.cu", "accumulate_ws3.cu", "synthesize.cu", "regular.cu", "burst.cu"]
+SOURCES = ["sim_api.cu", "accumulate.cu", "accumulate_ws3.cu", "synthesize.cu", "regular.cu", "burst.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
+              "-Xcompiler", "-fPIC", "-cudart", "shared"]
+
+
+def _deps():
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".h", ".cuh"))]
+    deps.append(os.path.join(INCLUDE, "sim.h"))
+    return deps
 
 
 def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".h", ".cuh"))]
-    deps.append(os.path.join(INCLUDE, "sim.h"))
-    return any(os.path.getmtime(d) > t for d in deps)
+    return any(os.path.getmtime(d) > t for d in _deps())
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
-        nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC]
+    if not (force or _stale()):
+        return LIB
+    nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    headers = [d for d in _deps() if not d.endswith(".cu")]
+    newest_header = max(os.path.getmtime(hd) for hd in headers)
+
+    def compile_one(src):
+        obj = os.path.join(OBJ, src[:-3] + ".o")
+        path = os.path.join(CSRC, src)
+        if (not force and os.path.exists(obj) and os.path.getmtime(obj) > os.path.getmtime(path)
+                and os.path.getmtime(obj) > newest_header):
+            return obj, ""
+        cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("SIM_NVCC_EXTRA", "").split(), "-I", INCLUDE, "-I", CSRC, "-c", path, "-o", obj]
         if verbose:
             cmd += ["-Xptxas", "-v"]
-        cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
-        subprocess.run(cmd, check=True)
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"nvcc failed on {src}:\n{r.stdout}\n{r.stderr}")
+        return obj, r.stderr
+
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    if verbose:
+        for _, log in results:
+            print(log)
+    subprocess.run([nvcc, "-shared", "-cudart", "shared", "-o", LIB, *[o for o, _ in results]], check=True)
     return LIB
 
 
 if __name__ == "__main__":
     import sys
-    print(build_lib(force=True, verbose="-v" in sys.argv))
+    print(build_lib(force="-f" in sys.argv or "-v" in sys.argv, verbose="-v" in sys.argv))

@@ -1,623 +1,714 @@
-// Steps A1-A7: scatterer -> (gate, Doppler bin, complex amplitude) -> spectrum T_u[G][N].
-// Paper: Algorithm 1 body and `rasterize`.  sm_100a, no tensor cores: the step is a
-// streaming scan (28 B per scatterer) with a scatter-add, bounded by HBM, the fp64 pipe and the
-// shared-memory atomic unit.  Design notes and measurements: DESIGN.md "Kernels".
+// Steps A1-A7: scatterers -> spectrum T_u[G][N] (Algorithm 1 body and `rasterize`).
+// sm_100a, no tensor cores: a streaming scan of 28 B per scatterer with a scatter-add, bounded by HBM bandwidth,
+// instruction issue and the shared-memory atomic unit.
+//
+// Production kernel `acc_kernel` (variant 4).  Persistent blocks, two per SM, NCW = 8 warps that all compute (128
+// registers per thread; a block of 9 or 10 warps gets 96):
+//   * scheduling units of consecutive scatterers are drawn from a global ticket counter (visited in a scattered order so
+//     that dark and illuminated parts of the scene are in flight together) and streamed in chunks of CH = NCW*32*PT
+//     through a ring of shared-memory stages by per-lane 16-byte asynchronous copies (cp.async.cg, LDGSTS: a warp
+//     instruction moves 512 contiguous bytes of one array).  There is no producer warp, no mbarrier and no hand-shake
+//     between warps on the load side: every lane copies exactly the 7 x 16 bytes it will read itself, one chunk ahead
+//     per extra stage, and waits for its own commit groups.  (Round 1 and the first versions of this kernel used TMA bulk
+//     copies issued by one lane per block or per warp: the uniform-register set-up of seven bulk copies per 4 KB slice
+//     cost more issue slots than it saved, and a refill that waits for the slowest warp of the block starved the fast
+//     ones.)  The sequence of chunks (base, count) is a small table in shared memory that whichever warp gets there
+//     first extends under a lock;
+//   * steps A2-A5 run in registers for IL scatterers at a time: range and phase in fp64 (polynomial in u = R^2 - rg0^2),
+//     Doppler coordinate in fp32 with a proven error bound, amplitude in fp32; gate, bin and the guard-band test are
+//     derived last, from two fixed-point integers, and the rare cases (guard band, outside the Doppler window, outside
+//     the fixed-point range) go through ONE cold block per group where the canonical fp64 sequence decides;
+//   * step A6 is block floating point: native int32 shared-memory reductions (red.shared.add.s32) of round(w c s) into a
+//     tile of FOUR planes [lower-gate half | upper-gate half] x [re | im], each [G+1][W]; s is a power of two fixed per
+//     epoch of <= 8191 scatterers from the geometric mean of the first warp's amplitudes, so that no cell can overflow.
+//     3 000-20 000 scatterers land in each hot cell and a warp's 32 scatterers hit only ~8 distinct cells, so same-address
+//     replays dominate the atomic unit; the four values of a scatterer are therefore issued in a lane-dependent order
+//     (lane bit 0 swaps re/im, lane bit 1 swaps lower/upper): every reduction instruction spreads its 32 lanes over all
+//     four planes and the replays per instruction drop from ~9.8 to ~6.5 (profiles/);
+//   * when the last warp has finished an epoch, every warp drains ITS SHARE of that epoch's gate rows into fp64 global
+//     reductions (step A7) at its next chunk boundary, while the second tile already fills with the next epoch: no drain
+//     warp, no rendez-vous, nobody falls behind by more than an eighth of a drain.  The global accumulator is an
+//     fp64 grid (exact enough that 10^5 identical escapes into one cell lose nothing); `acc_finalize_kernel` rounds it
+//     to the complex64 spectrum and re-zeroes it.
+// Reference kernel `acc_reference_kernel` (variant 0): one thread per scatterer, canonical sequence, global fp64
+// reductions; the A/B partner of the production kernel in the parity tests.
+// `sim_debug_indices` runs the production kernel itself with DBG = true (same index flow, indices written instead of
+// amplitudes accumulated).
 #include <climits>
 
-#include "sim_internal.h"
+#include "ptx_util.cuh"
+#include "scatter_math.cuh"
 
 namespace simk {
 
-// 1.5 * 2^(52 - kFracBits): adding it to v (|v| < 2^11) leaves floor/round(v * 2^20) in the low word.
-constexpr double kMagicFx = 6442450944.0;        // 1.5 * 2^32
-constexpr double kMagicFxHalf = 6442450944.5;    // the same + 0.5 (nearest-bin rule, ties up)
-constexpr double kMagicPhase = 402653184.0;      // 1.5 * 2^28: low word = round(q * 2^24)
-constexpr int kFxOne = 1 << kFracBits;
-constexpr float kFxScale = 1.0f / (float)kFxOne;
+constexpr int kAccMaxStages = 8;
+constexpr int kAccMaxWarps = 16;
+constexpr int kRing = 128;   // chunk table entries: more than two epochs (<= 2 * 31 chunks) + the stage ring
 
-struct Geo {
-  int g0, k;     // gate of the lower half in [-1, G-1], Doppler bin in [0, N)
-  float w1;      // weight of gate g0+1 (gate g0 gets 1 - w1)
-  float fr;      // frac(2R/lambda) mapped to [-0.5, 0.5) cycles
-  float delta;   // R - rg0, metres
+// epoch parameter slot (ring of 4): state, first bin of the Doppler window (unwrapped), scale exponent
+enum { kSlotState = 0, kSlotK0 = 1, kSlotEx = 2, kSlotInts = 4 };
+enum { kSlotUnset = 0, kSlotClaimed = 1, kSlotReady = 2 };
+// scheduling-unit table in shared memory (ring): first scatterer, end, sequence number (= unit index + 1 once published)
+int acc_chunk(int ncw, int pt) { return ncw * 32 * pt; }
+
+static int acc_row_stride(int W) { return (W + 3) & ~3; }   // words per tile row: 16-byte rows for the drain's vector loads
+
+size_t acc_tile_bytes(int G, int W) { return (size_t)4 * (G + 1) * acc_row_stride(W) * sizeof(int); }   // one tile: four planes
+
+size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages) {
+  return (size_t)stages * 7 * acc_chunk(ncw, pt) * sizeof(float) + 2 * acc_tile_bytes(G, W);
+}
+
+// A block works through scheduling units u = 0, 1, 2, ... (each a run of consecutive scatterers named by a ticket of the
+// global counter).  Unit u + `ahead` is prepared by the warp that is first to enter unit u: its lane 0 draws the ticket with an
+// asynchronous atomicAdd, keeps the value in a register while the reduction is in flight and publishes the unit (start,
+// end) at the end of its current chunk, long before anybody needs it.  Nobody spins on a lock; readers poll the
+// sequence number, all lanes together.
+struct PendingUnit {
+  unsigned ticket, unit;
+  bool pending;
 };
 
-__device__ __forceinline__ float phase_fraction(double two_over_lambda, double fr0, double delta) {
-  // 2R/lambda = 2 rg0/lambda + 2 delta/lambda; only the fraction matters (phase = -2 pi frac)
-  const double q = __fma_rn(delta, two_over_lambda, fr0);
-  const int lo = __double2loint(__dadd_rn(q, kMagicPhase));
-  return (float)(int)((unsigned)lo << 8) * 2.3283064365386963e-10f;  // * 2^-32
-}
-
-// ---------------------------------------------------------------------------------------------
-// CANONICAL fp64 INDEX SEQUENCE of DESIGN.md, continued from dx, dy, dz, R2 (which every path
-// computes identically).  Explicit round-to-nearest intrinsics: nvcc must not contract a*b+c
-// differently from the definition.  Kept out of line (the fast path calls it only inside the guard
-// band) and fed by value, so that the kernel parameters stay in constant memory.
-// Returns (g0, k, bits of w1, bits of fr); g0 = SIM_GATE_NONE when the scatterer is dropped.
-// ---------------------------------------------------------------------------------------------
-struct CanonConsts {
-  double rg0, inv_dR, cD, two_over_lambda, fr0, svx, svy, svz;
-  int G, N;
+struct UnitTable {
+  unsigned start0, end0, seq0;   // shared-memory addresses of the three rings
 };
 
-__device__ __noinline__ int4 canonical_tail(CanonConsts c, double dx, double dy, double dz, double R2,
-                                            float vxf, float vyf, float vzf) {
-  const int4 dropped = make_int4(SIM_GATE_NONE, -1, 0, 0);
-  const double R = __dsqrt_rn(R2);
-  const double delta = __dsub_rn(R, c.rg0);
-  const double gf = __dmul_rn(delta, c.inv_dR);
-  if (!(gf >= -1.0 && gf < (double)c.G)) return dropped;  // touches no gate (NaN lands here too)
-  const double g0d = floor(gf);
-  const double dvx = __dsub_rn((double)vxf, c.svx);
-  const double dvy = __dsub_rn((double)vyf, c.svy);
-  const double dvz = __dsub_rn((double)vzf, c.svz);
-  const double rdot = __ddiv_rn(__fma_rn(dvz, dz, __fma_rn(dvy, dy, __dmul_rn(dvx, dx))), R);
-  const double kf = __dmul_rn(rdot, c.cD);
-  if (!(fabs(kf) < 1073741824.0)) return dropped;
-  const double kk = floor(__dadd_rn(kf, 0.5));
-  // N is a power of two: two's-complement AND is the mathematical mod
-  return make_int4((int)g0d, ((int)kk) & (c.N - 1), __float_as_int((float)__dsub_rn(gf, g0d)),
-                   __float_as_int(phase_fraction(c.two_over_lambda, c.fr0, delta)));
-}
-
-__device__ __forceinline__ bool canonical(const AccParams& p, double dx, double dy, double dz, double R2,
-                                          float vxf, float vyf, float vzf, Geo& o) {
-  CanonConsts c;
-  c.rg0 = p.rg0; c.inv_dR = p.inv_dR; c.cD = p.cD; c.two_over_lambda = p.two_over_lambda; c.fr0 = p.fr0;
-  c.svx = p.svx; c.svy = p.svy; c.svz = p.svz; c.G = p.G; c.N = p.N;
-  const int4 r = canonical_tail(c, dx, dy, dz, R2, vxf, vyf, vzf);
-  if (r.x == SIM_GATE_NONE) return false;
-  o.g0 = r.x;
-  o.k = r.y;
-  o.w1 = __int_as_float(r.z);
-  o.fr = __int_as_float(r.w);
-  o.delta = ((float)r.x + o.w1) * p.dR_f;
-  return true;
-}
-
-// Steps A2-A4 of one scatterer.  Returns the packed indices (g0 + 1) | (k << 11), or -1 when the scatterer
-// touches no gate / is dropped; w1, fr and delta (fp32) are meaningful only for a non-negative code.
-//   FAST = false: the canonical sequence for every scatterer.
-//   FAST = true:  delta = R - rg0 from u = R^2 - rg0^2 by a 4-term series and 1/R by a 3-term series (no
-//   sqrt, no divide), gate and bin read from 2^-20 fixed point; whenever a coordinate lies within `guard`
-//   of a boundary the canonical sequence decides (bit-exact indices).
-// Written branch-free except for the rare guard-band call.
-template <bool FAST>
-__device__ __forceinline__ int geometry(const AccParams& p, float xf, float yf, float zf, float vxf,
-                                        float vyf, float vzf, float& w1, float& fr, float& delta_f,
-                                        unsigned& fallbacks) {
-  const double dx = __dsub_rn((double)xf, p.sx);
-  const double dy = __dsub_rn((double)yf, p.sy);
-  const double dz = __dsub_rn((double)zf, p.sz);
-  const double R2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-  if (!FAST) {
-    Geo g;
-    if (!canonical(p, dx, dy, dz, R2, vxf, vyf, vzf, g)) return -1;
-    w1 = g.w1; fr = g.fr; delta_f = g.delta;
-    return (g.g0 + 1) | (g.k << 11);
-  }
-  const double u = (R2 - p.rg0sq_hi) - p.rg0sq_lo;
-  const bool inwin = (u >= p.u_lo) && (u <= p.u_hi);  // false: certainly outside the window (or NaN)
-  const double t = u * p.inv_2rg0;
-  const double delta = t * fma(t, fma(t, fma(t, p.b3, p.b2), p.b1), 1.0);
-  const int gfx = __double2loint(__dadd_rd(delta * p.inv_dR, kMagicFx));   // floor(gf * 2^20)
-  const int gfrac = gfx & (kFxOne - 1);
-  const double dvx = (double)vxf - p.svx, dvy = (double)vyf - p.svy, dvz = (double)vzf - p.svz;
-  const double num = __fma_rn(dvz, dz, __fma_rn(dvy, dy, __dmul_rn(dvx, dx)));
-  const double e = delta * p.inv_rg0;
-  const double inv_R = p.inv_rg0 * fma(-e, fma(-e, 1.0 - e, 1.0), 1.0);   // 1/(rg0 (1+e)) to e^4
-  const double kf = (num * inv_R) * p.cD;
-  const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));             // floor((kf + 0.5) * 2^20)
-  const int kfrac = kfx & (kFxOne - 1);
-  const unsigned span = (unsigned)(kFxOne - 2 * p.guard);
-  const bool near = ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - p.guard) >= span) |
-                    !(fabs(kf) < 1024.0);
-  if (inwin && near) {  // rare: a coordinate sits in the guard band
-    ++fallbacks;
-    Geo g;
-    if (!canonical(p, dx, dy, dz, R2, vxf, vyf, vzf, g)) return -1;
-    w1 = g.w1; fr = g.fr; delta_f = g.delta;
-    return (g.g0 + 1) | (g.k << 11);
-  }
-  const int g0 = gfx >> kFracBits;
-  w1 = (float)gfrac * kFxScale;
-  fr = phase_fraction(p.two_over_lambda, p.fr0, delta);
-  delta_f = (float)gfx * p.dR_fx;
-  const bool ok = inwin & (g0 >= -1) & (g0 < p.G);
-  return ok ? ((g0 + 1) | (((kfx >> kFracBits) & (p.N - 1)) << 11)) : -1;
-}
-
-__device__ __forceinline__ float sqrt_approx(float v) {
-  float r;
-  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
-  return r;
-}
-__device__ __forceinline__ float ex2_approx(float v) {
-  float r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
-  return r;
-}
-
-// fp32 offsets from the satellite (hi + lo split of its position keeps the relative error at 2^-23)
-__device__ __forceinline__ void offsets_f32(const AccParams& p, float xf, float yf, float zf, float& dx,
-                                            float& dy, float& dz) {
-  dx = (xf - p.sxh) - p.sxl;
-  dy = (yf - p.syh) - p.syl;
-  dz = (zf - p.szh) - p.szl;
-}
-
-// Step A5: sqrt(s0dA) G(theta) / R^2 exp(-i 2 pi fr), all fp32.  Returns |c| too.
-__device__ __forceinline__ float2 amplitude(const AccParams& p, float dx, float dy, float dz, float delta_f,
-                                            float fr, float s0dA, float& A) {
-  const float e = delta_f * p.inv_rg0_f;
-  const float inv_R2 = p.inv_rg0sq_f * fmaf(e, fmaf(e, 3.0f, -2.0f), 1.0f);  // 1/(rg0 (1+e))^2 to e^3
-  const float cx = dy * p.bz - dz * p.by;
-  const float cy = dz * p.bx - dx * p.bz;
-  const float cz = dx * p.by - dy * p.bx;
-  const float sin2 = (cx * cx + cy * cy + cz * cz) * inv_R2;
-  A = sqrt_approx(s0dA) * ex2_approx(p.neg_alpha_log2e * sin2) * inv_R2;
-  float sn, cs;
-  __sincosf(6.283185307179586f * fr, &sn, &cs);
-  return make_float2(A * cs, -A * sn);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Variant 0: reference kernel.  One scatterer per thread, global fp32x2 reductions into T.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) acc_reference_kernel(AccParams p) {
-  const bool fast = p.index_path && p.fast_ok;
-  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  unsigned fb = 0;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n;
-       i += stride) {
-    const float s0 = p.s0dA[i];
-    if (!(s0 > 0.0f)) continue;
-    const float xf = p.x[i], yf = p.y[i], zf = p.z[i];
-    float w1, fr, df;
-    const int code = fast ? geometry<true>(p, xf, yf, zf, p.vx[i], p.vy[i], p.vz[i], w1, fr, df, fb)
-                          : geometry<false>(p, xf, yf, zf, p.vx[i], p.vy[i], p.vz[i], w1, fr, df, fb);
-    if (code < 0) continue;
-    const int g0 = (code & 2047) - 1, k = code >> 11;
-    float dx, dy, dz, A;
-    offsets_f32(p, xf, yf, zf, dx, dy, dz);
-    const float2 c = amplitude(p, dx, dy, dz, df, fr, s0, A);
-    const float w0 = 1.0f - w1;
-    if (g0 >= 0) atomicAdd(&p.T[(size_t)g0 * p.N + k], make_float2(w0 * c.x, w0 * c.y));
-    if (g0 + 1 < p.G) atomicAdd(&p.T[(size_t)(g0 + 1) * p.N + k], make_float2(w1 * c.x, w1 * c.y));
+__device__ __forceinline__ void publish_unit(const AccParams& p, const UnitTable& ut, unsigned long long n_sc, PendingUnit& t) {
+  if (t.pending) {
+    unsigned long long start = 0, end = 0;   // beyond the last ticket: an empty unit = end of work
+    if (t.ticket < n_sc) {
+      start = (((unsigned long long)t.ticket * p.sc_stride) % n_sc) * p.superchunk;   // tickets visit the scene in a scattered order
+      end = (start + p.superchunk < p.n) ? start + p.superchunk : p.n;
+    }
+    const unsigned slot = t.unit & (kRing - 1);
+    sh::st64(ut.start0 + 8u * slot, start);
+    sh::st64(ut.end0 + 8u * slot, end);
+    sh::st_release(ut.seq0 + 4u * slot, (int)(t.unit + 1u));
+    t.pending = false;
   }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Index-only kernel (parity pin P11): runs the same index routine as the production kernel.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) indices_kernel(AccParams p, int32_t* __restrict__ g0,
-                                                      int32_t* __restrict__ k) {
-  const bool fast = p.index_path && p.fast_ok;
-  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  unsigned fb = 0;
-  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n;
-       i += stride) {
-    float w1, fr, df;
-    const int code = fast ? geometry<true>(p, p.x[i], p.y[i], p.z[i], p.vx[i], p.vy[i], p.vz[i], w1, fr, df, fb)
-                          : geometry<false>(p, p.x[i], p.y[i], p.z[i], p.vx[i], p.vy[i], p.vz[i], w1, fr, df, fb);
-    g0[i] = code >= 0 ? (code & 2047) - 1 : SIM_GATE_NONE;
-    k[i] = code >= 0 ? (code >> 11) : -1;
-  }
-  if (fb) atomicAdd(&p.counters[kCtrFallback], fb);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Variant 1: shared-memory tile kernel (the production path).
-//
-//  * Persistent blocks draw "super-chunks" of consecutive scatterers from a ticket counter and stream them
-//    in chunks of CH = 256*PT.  Thread 0 is the scheduler/producer: it moves each chunk's seven 4*CH-byte
-//    array slices into a 2-stage shared-memory ring with TMA bulk copies (cp.async.bulk, completion on an
-//    mbarrier) two chunks ahead of use -- no registers are held by data in flight, no DRAM latency is
-//    exposed at a chunk or super-chunk boundary.
-//  * An fp32 pre-test (|u_f32 - u| <= 2^-21 R^2, margin 2^-20 R^2) discards the scatterers that are far
-//    outside the gate window before any fp64 work; a warp whose chunk is all outside skips phase 1.
-//  * sm_100a has no native shared-memory fp32 atomic add (it is an LDS + ATOMS.CAST.SPIN loop that
-//    collapses under the contention of this workload: 10^3..10^4 scatterers per populated cell), but
-//    ATOMS.ADD on int32 is native (measured 5 lanes/clk/SM whatever the contention).  Each chunk is
-//    therefore one block-floating-point EPOCH:
-//      phase 1  geometry + amplitude of the thread's PT scatterers, kept in registers; block statistics
-//               (count, mean amplitude, Doppler-offset range, gate range) by REDUX/shuffles + 5 ATOMS;
-//      phase 2  the Doppler window [k0, k0+W) is centred on the chunk's own bin range; contributions are
-//               scaled by s = 2^e with mean*s in [2^16, 2^17) and added with ATOMS.ADD to an int32 tile
-//               [G][W]; a component above 2^20 or a bin outside the window "escapes" to a global fp32x2
-//               reduction (exact, rare).  <= 1024 adds of <= 2^20 per cell: no overflow;
-//      drain    touched rows of the int tile x 2^-e -> global fp32x2 reductions into T (step A7), tile zeroed.
-//    Quantisation: LSB = 2^-e <= mean * 2^-16, so the relative L2 error of an epoch is <= 0.82 * 2^-16
-//    = 1.3e-5 whatever the amplitude distribution (mean <= rms); see DESIGN.md.
-// ---------------------------------------------------------------------------------------------
-namespace sh {  // shared-window addressing (32-bit shared addresses, computed once)
-__device__ __forceinline__ unsigned addr(const void* ptr) { return (unsigned)__cvta_generic_to_shared(ptr); }
-__device__ __forceinline__ void red_add(unsigned a, int v) {
-  asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-__device__ __forceinline__ void red_min(unsigned a, int v) {
-  asm volatile("red.shared.min.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-__device__ __forceinline__ void red_max(unsigned a, int v) {
-  asm volatile("red.shared.max.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-__device__ __forceinline__ int ld(unsigned a) {
-  int v;
-  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
-  return v;
-}
-__device__ __forceinline__ float ldf(unsigned a) {
-  float v;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st(unsigned a, int v) {
-  asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-__device__ __forceinline__ void stf(unsigned a, float v) {
-  asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
-}
-__device__ __forceinline__ int2 ld2(unsigned a) {
-  int2 v;
-  asm volatile("ld.shared.v2.s32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st2(unsigned a, int x, int y) {
-  asm volatile("st.shared.v2.s32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
-}
-template <int PT>
-__device__ __forceinline__ void ldv(unsigned a, float (&v)[PT]);
-template <>
-__device__ __forceinline__ void ldv<4>(unsigned a, float (&v)[4]) {
-  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(a) : "memory");
-}
-template <>
-__device__ __forceinline__ void ldv<2>(unsigned a, float (&v)[2]) {
-  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v[0]), "=f"(v[1]) : "r"(a) : "memory");
-}
-// mbarrier + TMA bulk copy (global -> shared, completion counted in bytes on the mbarrier)
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@!p bra WAIT_%=;\n\t}" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-               "l"(src), "r"(bytes), "r"(bar)
-               : "memory");
-}
-}  // namespace sh
-
-// per-chunk block statistics: 3 rotating sets of 8 ints + kAccWarps floats
-enum { kStDmin = 0, kStDmax, kStGmin, kStGmax, kStAnyk, kStCnt, kStInts = 8 };
-
-__device__ __forceinline__ void stats_reset(unsigned a) {
-  sh::st(a + 4 * kStDmin, INT_MAX);
-  sh::st(a + 4 * kStDmax, INT_MIN);
-  sh::st(a + 4 * kStGmin, INT_MAX);
-  sh::st(a + 4 * kStGmax, INT_MIN);
-  sh::st(a + 4 * kStAnyk, 0);
-  sh::st(a + 4 * kStCnt, 0);
-}
-
-// Scheduler state of thread 0: the sequence of chunks of this block.
-struct Cursor {
-  unsigned long long next, end;  // next chunk start, end of the current super-chunk
-  bool done;
-};
-
-// Thread 0: describe the next chunk of the block's sequence in slot `st` (base, valid count; count 0 = end of
-// work) and start its TMA copies.  Floats beyond the last whole group of four are left to the consumers.
-template <int CH>
-__device__ __forceinline__ void produce_chunk(const AccParams& p, Cursor& c, unsigned long long n_sc,
-                                              unsigned stage_smem, unsigned desc, unsigned bar) {
-  if (!c.done && c.next >= c.end) {
-    const unsigned long long sc = atomicAdd(&p.counters[kCtrTicket], 1u);
-    if (sc >= n_sc) {
-      c.done = true;
-    } else {
-      c.next = sc * p.superchunk;
-      c.end = (c.next + p.superchunk < p.n) ? c.next + p.superchunk : p.n;
+// Position of a chunk in the block's sequence: unit index and chunk index inside the unit; advanced chunk by chunk.
+struct ChunkPos {
+  unsigned unit, r;
+  __device__ __forceinline__ void advance(unsigned cps) {
+    if (++r == cps) {
+      r = 0;
+      ++unit;
     }
   }
-  unsigned nvalid = 0;
-  unsigned long long base = 0;
-  if (!c.done) {
-    base = c.next;
-    nvalid = (unsigned)((c.end - base < (unsigned long long)CH) ? c.end - base : CH);
-    c.next = base + nvalid;
+};
+
+// First scatterer and valid count of the chunk at `pos`; returns false at the end of work (an empty unit).  The last unit
+// of the scene may be short: its trailing chunks are empty (count 0) but not the end.  Called by all lanes together.
+template <int CH>
+__device__ __forceinline__ bool chunk_range(const UnitTable& ut, const ChunkPos& pos, unsigned long long& base, unsigned& nvalid) {
+  const unsigned slot = pos.unit & (kRing - 1);
+  while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != pos.unit + 1u) {
   }
-  asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(desc), "r"((unsigned)base), "r"((unsigned)(base >> 32)) : "memory");
-  sh::st(desc + 8, (int)nvalid);
-  const unsigned bytes = (nvalid & ~3u) * 4u;
-  sh::mbar_arrive_expect_tx(bar, 7u * bytes);  // release: the descriptor is visible to whoever sees the phase complete
-  if (bytes) {
-    const float* src[7] = {p.x, p.y, p.z, p.vx, p.vy, p.vz, p.s0dA};
-#pragma unroll
-    for (int a = 0; a < 7; ++a) sh::bulk_g2s(stage_smem + (unsigned)a * CH * 4u, src[a] + base, bytes, bar);
+  const unsigned long long start = sh::ld64(ut.start0 + 8u * slot), end = sh::ld64(ut.end0 + 8u * slot);
+  base = start + (unsigned long long)pos.r * CH;
+  nvalid = base < end ? (unsigned)((end - base < (unsigned long long)CH) ? end - base : CH) : 0u;
+  return end != 0ull;
+}
+
+// round(a * b) for |a b| <= 2^22 by the 1.5 * 2^23 trick (round to nearest even: unbiased), as an int
+__device__ __forceinline__ int fx_round(float a, float b) {
+  return __float_as_int(fmaf(a, b, 12582912.0f)) - 0x4B400000;
+}
+
+template <int PT>
+struct Vec;
+template <>
+struct Vec<2> {
+  float v[2];
+  __device__ __forceinline__ void load(unsigned a) {
+    const float2 t = sh::ldf2(a);
+    v[0] = t.x; v[1] = t.y;
+  }
+};
+template <>
+struct Vec<4> {
+  float v[4];
+  __device__ __forceinline__ void load(unsigned a) {
+    const float4 t = sh::ldf4(a);
+    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+  }
+};
+
+// true mod for the (rare) places that need the bin itself: N is any integer >= 1
+__device__ __forceinline__ int pmod(int a, int n) {
+  const int r = a % n;
+  return r < 0 ? r + n : r;
+}
+
+// One contribution that left the tile (or never used it): exact-enough fp64 global reductions.
+__device__ __forceinline__ void global_add(const AccParams& p, int g0, int k, float w1, float2 c) {
+  const int bin = pmod(k, p.N);
+  const double w1d = (double)w1, w0d = 1.0 - w1d;
+  if (g0 >= 0) {
+    double* t = reinterpret_cast<double*>(p.T64 + (size_t)g0 * p.N + bin);
+    atomicAdd(t, w0d * (double)c.x);
+    atomicAdd(t + 1, w0d * (double)c.y);
+  }
+  if (g0 + 1 < p.G) {
+    double* t = reinterpret_cast<double*>(p.T64 + (size_t)(g0 + 1) * p.N + bin);
+    atomicAdd(t, w1d * (double)c.x);
+    atomicAdd(t + 1, w1d * (double)c.y);
   }
 }
 
-template <int PT, int MB, bool FAST>
-__global__ void __launch_bounds__(kAccThreads, MB) acc_tile_kernel(AccParams p) {
-  constexpr int CH = kAccThreads * PT;
+template <int NCW, int PT, int IL, int MODE, bool DBG>
+__global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccParams p) {
+  constexpr int CH = NCW * 32 * PT, SL = 32 * PT;
   constexpr unsigned kStageBytes = 7u * CH * 4u;
+  constexpr unsigned kFull = 0xffffffffu;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ int s_stat[3][kStInts];
-  __shared__ float s_wsum[3][kAccWarps];
-  __shared__ __align__(8) unsigned long long s_bar[2];
-  __shared__ __align__(8) unsigned s_desc[2][4];
-
-  const int cells = p.G * p.W;
-  const unsigned stage0 = sh::addr(smem_raw);                 // 2 stages x 7 arrays x CH floats
-  const unsigned tile_i = stage0 + 2u * kStageBytes;           // int2 [G][W]
-  const unsigned stat0 = sh::addr(&s_stat[0][0]), wsum0 = sh::addr(&s_wsum[0][0]);
-  const unsigned bar0 = sh::addr(&s_bar[0]), desc0 = sh::addr(&s_desc[0][0]);
+  __shared__ __align__(8) unsigned long long s_ustart[kRing], s_uend[kRing];
+  __shared__ int s_useq[kRing];
+  __shared__ int s_claimed;             // units that some warp has entered (the first one in prepares unit + 2)
+  __shared__ int s_slot[4][kSlotInts];
+  __shared__ int s_tcount[2];           // warps that have finished the running epoch of tile b
+  __shared__ int s_complete[2];         // epochs of tile b that every warp has finished
+  __shared__ int s_shares[2];           // warps that have drained their share of the completed epoch of tile b
+  __shared__ int s_drained[2];          // epochs of tile b drained by every warp
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int N = p.N, W = p.W, halfW = W >> 1, halfN = N >> 1;
-  const int logW = 31 - __clz(W);
-  for (int c = tid; c < cells; c += kAccThreads) sh::st2(tile_i + 8u * c, 0, 0);
-  if (tid < 3) stats_reset(stat0 + 4u * kStInts * tid);
+  const int S = p.stages, EC = p.epoch_chunks;
+  const int G = p.G, W = p.W, RS = (W + 3) & ~3;
+  const unsigned stage0 = sh::addr(smem_raw);
+  const unsigned tile0 = stage0 + (unsigned)S * kStageBytes;     // int [2 tiles][4 planes: L.re, L.im, U.re, U.im][G + 1][RS]
+  const unsigned plane_bytes = (unsigned)((G + 1) * RS) * 4u, tile_bytes = 4u * plane_bytes;
+  const UnitTable ut{sh::addr(&s_ustart[0]), sh::addr(&s_uend[0]), sh::addr(&s_useq[0])};
+  const unsigned claimed_a = sh::addr(&s_claimed);
+  const unsigned tcount0 = sh::addr(&s_tcount[0]), drained0 = sh::addr(&s_drained[0]);
+  const unsigned complete0 = sh::addr(&s_complete[0]), shares0 = sh::addr(&s_shares[0]);
+  const unsigned slot0 = sh::addr(&s_slot[0][0]);
+  const unsigned cps = (unsigned)(p.superchunk / CH);          // chunks per scheduling unit
+  // the copies run S - 1 chunks ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
+  // need before the end of the chunk in which it is published
+  const unsigned ahead = ((unsigned)S - 1u + cps - 1u) / cps + 1u;
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
-  Cursor cursor{0, 0, false};
-  if (tid == 0) {
-    sh::mbar_init(bar0, 1);
-    sh::mbar_init(bar0 + 8, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    produce_chunk<CH>(p, cursor, n_sc, stage0, desc0, bar0);
-    produce_chunk<CH>(p, cursor, n_sc, stage0 + kStageBytes, desc0 + 16, bar0 + 8);
+  const unsigned e0 = (unsigned)lane * PT;             // this lane's first scatterer in the warp's slice
+  const unsigned slice_lo = (unsigned)warp * SL;       // the warp's slice in a chunk
+  const unsigned lane_smem = stage0 + (slice_lo + e0) * 4u;   // this lane's PT scatterers in stage 0, array 0
+
+  if (!DBG)
+    for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
+  for (int i = tid; i < kRing; i += NCW * 32) sh::st(ut.seq0 + 4u * i, 0);
+  if (tid < 4) sh::st(slot0 + 4u * kSlotInts * tid + 4 * kSlotState, kSlotUnset);
+  if (tid < 2) {
+    sh::st(tcount0 + 4u * tid, 0);
+    sh::st(drained0 + 4u * tid, 0);
+    sh::st(complete0 + 4u * tid, 0);
+    sh::st(shares0 + 4u * tid, 0);
+  }
+  __syncthreads();
+  if (tid == 0) {   // the first `ahead` units
+    sh::st(claimed_a, 0);
+    for (unsigned u = 0; u < ahead; ++u) {
+      PendingUnit t{atomicAdd(&p.counters[kCtrTicket], 1u), u, true};
+      publish_unit(p, ut, n_sc, t);
+    }
   }
   __syncthreads();
 
-  int kc = halfN;  // window centre of the previous chunk (reference of the signed circular Doppler offsets)
-  unsigned escapes = 0, fallbacks = 0;
-
-  for (unsigned chunk_no = 0;; ++chunk_no) {
-    const unsigned stg = chunk_no & 1u;
-    const unsigned stage = stage0 + stg * kStageBytes, desc = desc0 + 16u * stg, bar = bar0 + 8u * stg;
-    sh::mbar_wait(bar, (chunk_no >> 1) & 1u);
-    const unsigned nvalid = (unsigned)sh::ld(desc + 8);
-    if (nvalid == 0) break;  // block-uniform: end of work
-
-    // ---- this thread's PT scatterers: shared-memory stage -> registers ----
-    float x[PT], y[PT], z[PT], vx[PT], vy[PT], vz[PT], s0[PT];
-    const unsigned e0 = (unsigned)tid * PT;
-    if (e0 + PT <= (nvalid & ~3u)) {
-      const unsigned a = stage + e0 * 4u;
-      sh::ldv<PT>(a + 0u * CH * 4u, x);
-      sh::ldv<PT>(a + 1u * CH * 4u, y);
-      sh::ldv<PT>(a + 2u * CH * 4u, z);
-      sh::ldv<PT>(a + 3u * CH * 4u, vx);
-      sh::ldv<PT>(a + 4u * CH * 4u, vy);
-      sh::ldv<PT>(a + 5u * CH * 4u, vz);
-      sh::ldv<PT>(a + 6u * CH * 4u, s0);
-    } else {  // ragged end of the input: not covered by the 16-byte bulk copies; s0dA = 0 contributes nothing
-      unsigned long long base;
-      asm volatile("ld.shared.u64 %0, [%1];" : "=l"(base) : "r"(desc) : "memory");
-#pragma unroll
-      for (int j = 0; j < PT; ++j) {
-        const bool v = e0 + j < nvalid;
-        const unsigned long long i = base + e0 + j;
-        x[j] = v ? p.x[i] : 0.0f;
-        y[j] = v ? p.y[i] : 0.0f;
-        z[j] = v ? p.z[i] : 0.0f;
-        vx[j] = v ? p.vx[i] : 0.0f;
-        vy[j] = v ? p.vy[i] : 0.0f;
-        vz[j] = v ? p.vz[i] : 0.0f;
-        s0[j] = v ? p.s0dA[i] : 0.0f;
-      }
+  PendingUnit tk{0u, 0u, false};
+  // This lane's PT scatterers of the chunk at `pos` (7 x 16 bytes) -> its place in stage `st`; one commit group per chunk,
+  // empty beyond the end of the input.  PT = 2 lanes pair up: the even lane copies for both.
+  auto copy_chunk = [&](const ChunkPos& pos, unsigned st) {
+    unsigned long long base;
+    unsigned nv;
+    chunk_range<CH>(ut, pos, base, nv);
+    const unsigned n4 = nv & ~3u;
+    const unsigned o4 = (slice_lo + e0) & ~3u;                    // first scatterer of this lane's 16-byte group
+    if ((PT == 4 || !(lane & 1)) && o4 + 4u <= n4) {
+      const unsigned dst = stage0 + st * kStageBytes + o4 * 4u;
+      const unsigned long long g = base + o4;
+      sh::cp_async16(dst + 0u * CH * 4u, p.x + g);
+      sh::cp_async16(dst + 1u * CH * 4u, p.y + g);
+      sh::cp_async16(dst + 2u * CH * 4u, p.z + g);
+      sh::cp_async16(dst + 3u * CH * 4u, p.vx + g);
+      sh::cp_async16(dst + 4u * CH * 4u, p.vy + g);
+      sh::cp_async16(dst + 5u * CH * 4u, p.vz + g);
+      sh::cp_async16(dst + 6u * CH * 4u, p.s0dA + g);
     }
-
-    // ---- phase 1: geometry + amplitude in registers, block statistics ----
-    int code[PT];
-    float w1[PT], re[PT], im[PT];
-    float dxf[PT], dyf[PT], dzf[PT];
-    bool maybe = false;
-#pragma unroll
-    for (int j = 0; j < PT; ++j) {
-      offsets_f32(p, x[j], y[j], z[j], dxf[j], dyf[j], dzf[j]);
-      const float uf = fmaf(dzf[j], dzf[j], fmaf(dyf[j], dyf[j], dxf[j] * dxf[j])) - p.rg0sq_f;
-      // s0dA <= 0 or NaN: dead.  Pre-test: certainly outside the window (NaN position lands here too).
-      const bool live_j = (s0[j] > 0.0f) && (!FAST || (uf >= p.uf_lo && uf <= p.uf_hi));
-      code[j] = live_j ? 0 : -1;
-      maybe |= live_j;
-    }
-    int cnt = 0, dmin = INT_MAX, dmax = INT_MIN, gmin = INT_MAX, gmax = INT_MIN, anyk = 0;
-    float sumA = 0.0f;
-    if (__any_sync(0xffffffffu, maybe)) {  // warp-uniform: skip warps that are entirely dark
-#pragma unroll
-      for (int j = 0; j < PT; ++j) {
-        if (code[j] < 0) continue;
-        float fr, df;
-        code[j] = geometry<FAST>(p, x[j], y[j], z[j], vx[j], vy[j], vz[j], w1[j], fr, df, fallbacks);
-        float A;
-        const float2 c = amplitude(p, dxf[j], dyf[j], dzf[j], df, fr, s0[j], A);
-        re[j] = c.x;
-        im[j] = c.y;
-        const bool ok = code[j] >= 0;
-        const int k = code[j] >> 11, g0 = (code[j] & 2047) - 1;
-        const int d = ((k - kc + halfN) & (N - 1)) - halfN;  // signed circular offset from the last centre
-        dmin = min(dmin, ok ? d : INT_MAX);
-        dmax = max(dmax, ok ? d : INT_MIN);
-        gmin = min(gmin, ok ? g0 : INT_MAX);
-        gmax = max(gmax, ok ? g0 : INT_MIN);
-        anyk = ok ? k : anyk;
-        cnt += ok ? 1 : 0;
-        sumA += ok ? A : 0.0f;
-      }
-    }
-    const unsigned st = stat0 + 4u * kStInts * (chunk_no % 3u);
-    const unsigned wsum = wsum0 + 4u * kAccWarps * (chunk_no % 3u);
-    const unsigned live = __ballot_sync(0xffffffffu, cnt > 0);
-    if (live) {  // warp-uniform
-      dmin = __reduce_min_sync(0xffffffffu, dmin);
-      dmax = __reduce_max_sync(0xffffffffu, dmax);
-      gmin = __reduce_min_sync(0xffffffffu, gmin);
-      gmax = __reduce_max_sync(0xffffffffu, gmax);
-      cnt = __reduce_add_sync(0xffffffffu, cnt);
-      anyk = __shfl_sync(0xffffffffu, anyk, __ffs(live) - 1);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) sumA += __shfl_xor_sync(0xffffffffu, sumA, o);
-      if (lane == 0) {
-        sh::red_min(st + 4 * kStDmin, dmin);
-        sh::red_max(st + 4 * kStDmax, dmax);
-        sh::red_min(st + 4 * kStGmin, gmin);
-        sh::red_max(st + 4 * kStGmax, gmax);
-        sh::red_add(st + 4 * kStCnt, cnt);
-        sh::st(st + 4 * kStAnyk, anyk);
-      }
-    }
-    if (lane == 0) sh::stf(wsum + 4u * warp, live ? sumA : 0.0f);
-    __syncthreads();  // (A) statistics complete; stage `stg` fully read; every drain of the previous chunk done
-    if (tid == 0) {
-      // the set read one chunk ago is next written after the next (A): safe to reset now
-      stats_reset(stat0 + 4u * kStInts * ((chunk_no + 2u) % 3u));
-      produce_chunk<CH>(p, cursor, n_sc, stage, desc, bar);  // chunk_no + 2 into the stage just consumed
-    }
-
-    const int tot = sh::ld(st + 4 * kStCnt);
-    if (tot == 0) continue;  // block-uniform: nothing illuminated in this chunk
-
-    // ---- Doppler window of this epoch, centred on the chunk's own bin range ----
-    const int bdmin = sh::ld(st + 4 * kStDmin), bdmax = sh::ld(st + 4 * kStDmax);
-    if (W < N) kc = ((bdmax - bdmin < W) ? kc + ((bdmin + bdmax + 1) >> 1) : sh::ld(st + 4 * kStAnyk)) & (N - 1);
-    const int k0 = (kc - halfW) & (N - 1);
-
-    // ---- block-floating-point scale of this epoch: mean * s in [2^16, 2^17) ----
-    float tsum = 0.0f;
-#pragma unroll
-    for (int w = 0; w < kAccWarps; ++w) tsum += sh::ldf(wsum + 4u * w);
-    const float mean = tsum / (float)tot;
-    int ex = 16 - (((__float_as_int(mean) >> 23) & 0xff) - 127);
-    ex = max(-126, min(127, ex));
-    const float s = __int_as_float((ex + 127) << 23);
-    const float inv_s = __int_as_float((127 - ex) << 23);
-    const float lim = 1048575.0f * inv_s;  // |component| * s <= 2^20 - 1
-
-    // ---- phase 2: native int32 shared-memory atomics ----
-    bool esc_any = false;
-#pragma unroll
-    for (int j = 0; j < PT; ++j) {
-      const int k = code[j] >> 11, g0 = (code[j] & 2047) - 1;
-      const unsigned kw = (unsigned)(k - k0) & (unsigned)(N - 1);
-      const bool ok = code[j] >= 0;
-      const bool fits = ok && kw < (unsigned)W && fmaxf(fabsf(re[j]), fabsf(im[j])) <= lim;
-      const float w1s = w1[j] * s, w0s = s - w1s;
-      // round(v * s) by the 1.5 * 2^23 trick (|v * s| <= 2^20): low mantissa bits, bias removed
-      const unsigned a0 = tile_i + 8u * (unsigned)((g0 << logW) + (int)kw);
-      if (fits && g0 >= 0) {
-        sh::red_add(a0, __float_as_int(fmaf(re[j], w0s, 12582912.0f)) - 0x4B400000);
-        sh::red_add(a0 + 4, __float_as_int(fmaf(im[j], w0s, 12582912.0f)) - 0x4B400000);
-      }
-      if (fits && g0 + 1 < p.G) {
-        const unsigned a1 = a0 + 8u * (unsigned)W;
-        sh::red_add(a1, __float_as_int(fmaf(re[j], w1s, 12582912.0f)) - 0x4B400000);
-        sh::red_add(a1 + 4, __float_as_int(fmaf(im[j], w1s, 12582912.0f)) - 0x4B400000);
-      }
-      code[j] = (ok && !fits) ? code[j] : -1;  // what is left escapes
-      esc_any |= (ok && !fits);
-    }
-    if (__any_sync(0xffffffffu, esc_any)) {  // rare
-#pragma unroll
-      for (int j = 0; j < PT; ++j) {
-        if (code[j] < 0) continue;
-        const int k = code[j] >> 11, g0 = (code[j] & 2047) - 1;
-        const float w0 = 1.0f - w1[j];
-        if (g0 >= 0) atomicAdd(&p.T[(size_t)g0 * N + k], make_float2(w0 * re[j], w0 * im[j]));
-        if (g0 + 1 < p.G) atomicAdd(&p.T[(size_t)(g0 + 1) * N + k], make_float2(w1[j] * re[j], w1[j] * im[j]));
-        ++escapes;
-      }
-    }
-    __syncthreads();  // (B) all atomics of the epoch landed
-
-    // ---- drain (step A7): touched rows of the int tile -> global fp32x2 reductions ----
-    const int r0 = max(sh::ld(st + 4 * kStGmin), 0), r1 = min(sh::ld(st + 4 * kStGmax) + 1, p.G - 1);
-    const int dbase = r0 << logW, dcells = (r1 - r0 + 1) << logW;
-    for (int cc = tid; cc < dcells; cc += kAccThreads) {
-      const int c = dbase + cc;
-      const int2 v = sh::ld2(tile_i + 8u * (unsigned)c);
-      if (v.x | v.y) {
-        sh::st2(tile_i + 8u * (unsigned)c, 0, 0);
-        const int g = c >> logW, kw = c & (W - 1);
-        atomicAdd(&p.T[(size_t)g * N + ((k0 + kw) & (N - 1))], make_float2((float)v.x * inv_s, (float)v.y * inv_s));
-      }
-    }
+    sh::cp_async_commit();
+  };
+  ChunkPos cpos{0u, 0u};   // the chunk to copy next
+  ChunkPos rpos{0u, 0u};   // the chunk to read next
+  for (int s = 0; s + 1 < S; ++s) {   // chunks 0 .. S-2 are in flight
+    copy_chunk(cpos, (unsigned)s);
+    cpos.advance(cps);
   }
 
+  // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
+  // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
+  // halves of row g (g0 = g - 1); row 0 of L and row G of U only collect the halves that fall outside the window: never
+  // read, never zeroed.  One lane = four consecutive bins of one gate: four 16-byte loads.
+  const int g_lo = (int)(((long long)G * warp) / NCW), g_hi = (int)(((long long)G * (warp + 1)) / NCW);
+  const int quads = RS >> 2;
+  auto drain_share = [&](unsigned d) {
+    const unsigned b = d & 1u;
+    const unsigned slot = slot0 + 4u * kSlotInts * (d & 3u);
+    if (sh::ld(slot + 4 * kSlotState) == kSlotReady) {
+      const int k0 = pmod(sh::ld(slot + 4 * kSlotK0), p.N), ex = sh::ld(slot + 4 * kSlotEx);
+      const double inv_s = __hiloint2double((1023 - ex) << 20, 0);
+      const unsigned tile = tile0 + b * tile_bytes;
+      const int nitem = (g_hi - g_lo) * quads;
+      for (int it = lane; it < nitem; it += 32) {
+        const int g = g_lo + it / quads, q4 = (it % quads) * 4;
+        const unsigned aL = tile + 4u * (unsigned)((g + 1) * RS + q4), aU = tile + 2u * plane_bytes + 4u * (unsigned)(g * RS + q4);
+        const int4 lr = sh::ld4(aL), li = sh::ld4(aL + plane_bytes), ur = sh::ld4(aU), ui = sh::ld4(aU + plane_bytes);
+        const int any = lr.x | lr.y | lr.z | lr.w | li.x | li.y | li.z | li.w | ur.x | ur.y | ur.z | ur.w | ui.x | ui.y | ui.z | ui.w;
+        if (any) {
+          const int4 z4 = make_int4(0, 0, 0, 0);
+          sh::st4(aL, z4);
+          sh::st4(aL + plane_bytes, z4);
+          sh::st4(aU, z4);
+          sh::st4(aU + plane_bytes, z4);
+          const int re[4] = {lr.x + ur.x, lr.y + ur.y, lr.z + ur.z, lr.w + ur.w};
+          const int im[4] = {li.x + ui.x, li.y + ui.y, li.z + ui.z, li.w + ui.w};
+  #pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            if (re[c] | im[c]) {   // (columns >= W are never written)
+              int bin = k0 + q4 + c;
+              bin -= bin >= p.N ? p.N : 0;
+              double* t = reinterpret_cast<double*>(p.T64 + (size_t)g * p.N + bin);
+              atomicAdd(t, (double)re[c] * inv_s);
+              atomicAdd(t + 1, (double)im[c] * inv_s);
+            }
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0 && sh::atom_add_acq_rel(shares0 + 4u * b, 1) == NCW - 1) {   // every share is out: tile and slot go back
+      sh::st(shares0 + 4u * b, 0);
+      sh::st(slot + 4 * kSlotState, kSlotUnset);
+      sh::st_release(drained0 + 4u * b, (int)(d >> 1) + 1);
+    }
+    __syncwarp();
+  };
+  // Drains the shares of the epochs before `upto` that are complete; called at chunk boundaries (cheap when nothing is
+  // pending).  block = true: waits for the completion (end of the kernel, or a tile that this warp needs back).
+  unsigned dpend = 0;   // the oldest epoch whose share this warp has not drained yet
+  auto try_drain = [&](unsigned upto, bool block) {
+    while (dpend < upto) {
+      const unsigned b = dpend & 1u;
+      if (sh::ld_acquire(complete0 + 4u * b) <= (int)(dpend >> 1)) {
+        if (!block) return;
+        continue;
+      }
+      drain_share(dpend);
+      ++dpend;
+    }
+  };
+
+  // lane-dependent issue order of a scatterer's four reductions: bit 0 swaps re/im, bit 1 swaps lower/upper
+  const bool sw_ri = lane & 1, sw_lu = (lane >> 1) & 1;
+  const unsigned off_b0 = (sw_lu ? 2u : 0u) * plane_bytes + (sw_ri ? plane_bytes : 0u);   // plane of (value a0, weight wB)
+  const int d_ri = sw_ri ? -(int)plane_bytes : (int)plane_bytes;                          // a0 -> a1
+  const int d_lu = sw_lu ? -2 * (int)plane_bytes : 2 * (int)plane_bytes;                  // wB -> wA
+  const int RS4 = 4 * RS;
+  unsigned stg = 0;
+  unsigned escapes = 0, fallbacks = 0;
+  bool more = true;
+  const unsigned fx_span = (unsigned)(p.fx_cap - 11) << 23;   // admitted |c| s: [2^11, 2^fx_cap]
+
+  for (unsigned e = 0; more; ++e) {
+    const unsigned slot = slot0 + 4u * kSlotInts * (e & 3u);
+    if (!DBG && e >= 2) {   // the tile of epoch e-2 must be back: this warp's own share first, then everybody else's
+      try_drain(e - 1u, true);
+      while (sh::ld_acquire(drained0 + 4u * (e & 1u)) < (int)(e >> 1)) {
+      }
+    }
+    // tile base of this lane's first reduction, the +1 row offset of the padded tile folded in
+    const unsigned tile_b = tile0 + (e & 1u) * tile_bytes + (unsigned)RS4 + off_b0;
+    bool have = false;         // this warp holds the epoch's parameters
+    int k0 = 0, lo_bits = 0;
+    float s = 0.0f, sS = 0.0f, sO = 0.0f;
+    int ci = 0;
+    for (; ci < EC; ++ci) {
+      if (!DBG && dpend < e) try_drain(e, false);
+      // chunk cidx + S - 1 goes into the stage that was read one iteration ago; then this lane's copies of chunk cidx
+      // (S - 1 groups older) must have landed
+      copy_chunk(cpos, stg == 0 ? (unsigned)S - 1u : stg - 1u);
+      cpos.advance(cps);
+      switch (S) {
+        case 2: sh::cp_async_wait<1>(); break;
+        case 3: sh::cp_async_wait<2>(); break;
+        case 4: sh::cp_async_wait<3>(); break;
+        case 5: sh::cp_async_wait<4>(); break;
+        case 6: sh::cp_async_wait<5>(); break;
+        case 7: sh::cp_async_wait<6>(); break;
+        default: sh::cp_async_wait<7>(); break;
+      }
+      if (PT == 2) __syncwarp();   // the even lane's copy serves its odd neighbour
+      unsigned long long base;
+      unsigned nvalid;
+      if (!chunk_range<CH>(ut, rpos, base, nvalid)) {   // block-uniform: end of work
+        more = false;
+        break;
+      }
+      if (rpos.r == 0) {   // the first warp to enter a unit prepares a later one
+        if (lane == 0 && sh::cas(claimed_a, (int)rpos.unit, (int)rpos.unit + 1) == (int)rpos.unit) {
+          tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
+          tk.unit = rpos.unit + ahead;
+          tk.pending = true;
+        }
+        __syncwarp();
+      }
+      rpos.advance(cps);
+
+      // ---- step A1: this lane's PT scatterers, shared-memory stage -> registers; the slice is refilled at once ----
+      Vec<PT> x, y, z, vx, vy, vz, s0;
+      const unsigned off = slice_lo + e0;         // offset in the chunk
+      if (off + PT <= (nvalid & ~3u)) {
+        const unsigned a = lane_smem + stg * kStageBytes;
+        x.load(a + 0u * CH * 4u);
+        y.load(a + 1u * CH * 4u);
+        z.load(a + 2u * CH * 4u);
+        vx.load(a + 3u * CH * 4u);
+        vy.load(a + 4u * CH * 4u);
+        vz.load(a + 5u * CH * 4u);
+        s0.load(a + 6u * CH * 4u);
+      } else {  // ragged end of the input: not covered by the 16-byte bulk copies; s0dA = 0 contributes nothing
+#pragma unroll
+        for (int j = 0; j < PT; ++j) {
+          const bool v = off + j < nvalid;
+          const unsigned long long i = base + off + j;
+          x.v[j] = v ? p.x[i] : 0.0f;
+          y.v[j] = v ? p.y[i] : 0.0f;
+          z.v[j] = v ? p.z[i] : 0.0f;
+          vx.v[j] = v ? p.vx[i] : 0.0f;
+          vy.v[j] = v ? p.vy[i] : 0.0f;
+          vz.v[j] = v ? p.vz[i] : 0.0f;
+          s0.v[j] = v ? p.s0dA[i] : 0.0f;
+        }
+      }
+      if (++stg == (unsigned)S) stg = 0;
+
+#pragma unroll
+      for (int gi = 0; gi < PT; gi += IL) {   // IL scatterers in flight per lane at a time
+        // ---- steps A2-A5 ----
+        bool ok[IL];
+        Pre q[IL];
+        Fx fx[IL];
+        float2 c[IL];
+        int ab[IL];
+        bool any = false;
+  #pragma unroll
+        for (int j = 0; j < IL; ++j) {
+          ok[j] = DBG ? (off + gi + j < nvalid) : (s0.v[gi + j] > 0.0f);   // s0dA <= 0 or NaN: dead (not consulted by the index export)
+          q[j] = pre_part<MODE>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], ok[j]);
+          any |= ok[j];
+        }
+        if (!__any_sync(kFull, any)) {   // warp-uniform: the whole warp is dark
+          if (DBG) {
+  #pragma unroll
+            for (int j = 0; j < IL; ++j)
+              if (off + gi + j < nvalid) {
+                p.dbg_g0[base + off + gi + j] = SIM_GATE_NONE;
+                p.dbg_k[base + off + gi + j] = -1;
+              }
+          }
+          continue;
+        }
+        Idx cx[IL];   // canonical mode only
+        if (MODE == kIdxCanonical) {
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) {
+            ok[j] = ok[j] && canonical(p, q[j].dx, q[j].dy, q[j].dz, vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], cx[j]);
+            // g0 and a 20-bit weight for the tile path; the bin itself (no fraction bits)
+            fx[j].gfx = (cx[j].g0 << kFracBits) + min((int)(cx[j].w1 * (float)kFxOne), kFxOne - 1);
+            fx[j].kfx = cx[j].k;
+            fx[j].fr = cx[j].fr;
+          }
+        } else {
+          // polynomial path straight through for all IL scatterers; the guard-band cases are re-decided in the cold block
+  #pragma unroll
+          for (int j = 0; j < IL; ++j)
+            fx[j] = index_fx<MODE>(p, q[j], x.v[gi + j], y.v[gi + j], z.v[gi + j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j]);
+        }
+        if (!DBG) {
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) {
+            float A;
+            c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr, s0.v[gi + j], A);
+            ab[j] = __float_as_int(A);
+          }
+        }
+        // ---- gate, bin, weight and the guard-band test, from the two fixed-point coordinates ----
+        int g0[IL], k[IL];
+        bool near[IL];
+        any = false;
+  #pragma unroll
+        for (int j = 0; j < IL; ++j) {
+          g0[j] = fx[j].gfx >> kFracBits;
+          if (MODE == kIdxCanonical) {
+            k[j] = fx[j].kfx;
+            near[j] = false;
+          } else {
+            k[j] = fx_bin<MODE>(p, fx[j]);
+            near[j] = ok[j] && fx_near<MODE>(p, fx[j]);
+          }
+          any |= ok[j];
+        }
+        if (DBG) {
+          bool any_near = false;
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) any_near |= near[j];
+          if (__any_sync(kFull, any_near)) {
+  #pragma unroll
+            for (int j = 0; j < IL; ++j) {
+              if (near[j]) {
+                ++fallbacks;
+                Idx t;
+                ok[j] = canonical(p, __dsub_rn((double)x.v[gi + j], p.sx), __dsub_rn((double)y.v[gi + j], p.sy),
+                                  __dsub_rn((double)z.v[gi + j], p.sz), vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], t);
+                g0[j] = t.g0;
+                k[j] = t.k;
+              }
+            }
+          }
+  #pragma unroll
+          for (int j = 0; j < IL; ++j)
+            if (off + gi + j < nvalid) {
+              p.dbg_g0[base + off + gi + j] = ok[j] ? g0[j] : SIM_GATE_NONE;
+              p.dbg_k[base + off + gi + j] = ok[j] ? pmod(k[j], p.N) : -1;
+            }
+          continue;
+        }
+        const unsigned okm = __ballot_sync(kFull, any);
+        if (okm == 0) continue;
+
+        // ---- epoch parameters: the first warp with something to add decides them ----
+        if (!have) {
+          int st = 0;
+          if (lane == 0) {
+            st = sh::ld_acquire(slot + 4 * kSlotState);
+            if (st != kSlotReady) st = sh::cas(slot + 4 * kSlotState, kSlotUnset, kSlotClaimed);
+          }
+          st = __shfl_sync(kFull, st, 0);
+          if (st == kSlotUnset) {  // this warp won the claim: window and scale from its own scatterers
+            int kk = 0;
+  #pragma unroll
+            for (int j = IL - 1; j >= 0; --j) kk = ok[j] ? k[j] : kk;
+            const int kref = __shfl_sync(kFull, kk, __ffs(okm) - 1);
+            int dmin = INT_MAX, dmax = INT_MIN, cnt = 0, slog = 0;
+  #pragma unroll
+            for (int j = 0; j < IL; ++j) {
+              const int d = k[j] - kref;                                     // bins are unwrapped here: plain offsets
+              dmin = min(dmin, ok[j] ? d : INT_MAX);
+              dmax = max(dmax, ok[j] ? d : INT_MIN);
+              cnt += ok[j] ? 1 : 0;
+              slog += ok[j] ? (ab[j] >> 16) : 0;                            // log2 amplitude, 2^-7 units
+            }
+            dmin = __reduce_min_sync(kFull, dmin);
+            dmax = __reduce_max_sync(kFull, dmax);
+            cnt = __reduce_add_sync(kFull, cnt);
+            slog = __reduce_add_sync(kFull, slog);
+            if (lane == 0) {
+              const int centre = ((long long)dmax - dmin < W) ? kref + ((dmin + dmax + 1) >> 1) : kref;
+              const int E = (slog / cnt) >> 7;                      // biased exponent of the geometric mean
+              const int ex = max(-100, min(120, p.fx_target - (E - 127)));   // gmean * 2^ex in [2^16, 2^17) (default)
+              sh::st(slot + 4 * kSlotK0, centre - (W >> 1));
+              sh::st(slot + 4 * kSlotEx, ex);
+              sh::st_release(slot + 4 * kSlotState, kSlotReady);
+            }
+            __syncwarp();
+          } else if (st == kSlotClaimed) {
+            while (sh::ld_acquire(slot + 4 * kSlotState) != kSlotReady) {
+            }
+          }
+          k0 = sh::ld(slot + 4 * kSlotK0);
+          const int ex = sh::ld(slot + 4 * kSlotEx);
+          s = __int_as_float((ex + 127) << 23);
+          sS = sw_lu ? -s : s;
+          sO = sw_lu ? s : 0.0f;
+          lo_bits = (11 - ex + 127) << 23;                    // bits of 2^11 / s
+          have = true;
+        }
+
+        // ---- step A6: native int32 shared-memory reductions; whatever does not fit takes the cold block ----
+        bool slow_any = false;
+        bool slow[IL];
+  #pragma unroll
+        for (int j = 0; j < IL; ++j) {
+          const int kw = k[j] - k0;
+          const bool fits = ok[j] && !near[j] && (unsigned)kw < (unsigned)W && (unsigned)(ab[j] - lo_bits) <= fx_span;
+          const float w1 = (float)(fx[j].gfx & (kFxOne - 1)) * p.w_scale;
+          const float wAs = fmaf(w1, sS, sO), wBs = s - wAs;             // (w1, w0) s, or (w0, w1) s on swapped lanes
+          const float a0 = sw_ri ? c[j].y : c[j].x, a1 = sw_ri ? c[j].x : c[j].y;
+          const unsigned adr = tile_b + (unsigned)(g0[j] * RS4 + 4 * kw);
+          if (fits) {
+            sh::red_add(adr, fx_round(a0, wBs));
+            sh::red_add(adr + d_ri, fx_round(a1, wBs));
+            sh::red_add(adr + d_lu, fx_round(a0, wAs));
+            sh::red_add(adr + d_lu + d_ri, fx_round(a1, wAs));
+          }
+          slow[j] = ok[j] && !fits;
+          slow_any |= slow[j];
+        }
+        if (__any_sync(kFull, slow_any)) {  // rare: guard band (canonical sequence decides), window or range escape
+  #pragma unroll
+          for (int j = 0; j < IL; ++j) {
+            if (slow[j]) {
+              Idx t;
+              if (MODE == kIdxCanonical) {
+                t = cx[j];
+              } else {
+                if (near[j]) ++fallbacks;
+                // the canonical sequence for every scatterer that leaves the tile (guard band or not: it is exact);
+                // offsets recomputed here (three subtractions) rather than kept alive across the amplitude for this rare case
+                const bool okj = canonical(p, __dsub_rn((double)x.v[gi + j], p.sx), __dsub_rn((double)y.v[gi + j], p.sy),
+                                           __dsub_rn((double)z.v[gi + j], p.sz), vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], t);
+                if (!okj) continue;
+                float A;
+                c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], t.gfx, t.fr, s0.v[gi + j], A);
+              }
+              global_add(p, t.g0, t.k, t.w1, c[j]);
+              ++escapes;
+            }
+          }
+        }
+      }
+      // the ticket drawn when this warp was first into a unit (at the top of this chunk) has had the whole chunk to come
+      // back: the unit is published before this warp can wait for anybody
+      if (lane == 0) publish_unit(p, ut, n_sc, tk);
+      __syncwarp();
+    }
+
+    // ---- end of an epoch (or of the input inside one): the last warp out declares the tile complete ----
+    if (!DBG) {
+      __syncwarp();
+      if (lane == 0 && sh::atom_add_acq_rel(tcount0 + 4u * (e & 1u), 1) == NCW - 1) {
+        sh::st(tcount0 + 4u * (e & 1u), 0);
+        sh::st_release(complete0 + 4u * (e & 1u), (int)(e >> 1) + 1);
+      }
+      __syncwarp();
+      if (!more) try_drain(e + 1u, true);   // the end of the input: the shares of the last epochs
+    }
+  }
+  if (lane == 0) publish_unit(p, ut, n_sc, tk);
   if (escapes) atomicAdd(&p.counters[kCtrEscape], escapes);
   if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
 }
 
 // ---------------------------------------------------------------------------------------------
+// Variant 0: reference kernel.  One scatterer per thread, the canonical sequence for every scatterer, fp64 global
+// reductions.  Plain on purpose: it is the A/B partner of the production kernel.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) acc_reference_kernel(AccParams p) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.n; i += stride) {
+    const float s0 = p.s0dA[i];
+    if (!(s0 > 0.0f)) continue;
+    const float xf = p.x[i], yf = p.y[i], zf = p.z[i];
+    Idx ix;
+    if (!canonical(p, __dsub_rn((double)xf, p.sx), __dsub_rn((double)yf, p.sy), __dsub_rn((double)zf, p.sz), p.vx[i], p.vy[i],
+                   p.vz[i], ix))
+      continue;
+    float A;
+    const float2 c = amplitude(p, xf, yf, zf, ix.gfx, ix.fr, s0, A);
+    global_add(p, ix.g0, ix.k, ix.w1, c);
+  }
+}
+
+// T64 -> spectrum slot (complex64), T64 re-zeroed.  add != 0: the slot already holds earlier batches of this update
+// (SIM_ACC_APPEND).
+__global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= cells) return;
+  const double2 v = T64[i];
+  float2 o = make_float2((float)v.x, (float)v.y);
+  if (add) {
+    const float2 t = T[i];
+    o.x += t.x;
+    o.y += t.y;
+  }
+  T[i] = o;
+  if (v.x != 0.0 || v.y != 0.0) T64[i] = make_double2(0.0, 0.0);
+}
+
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches) {
+  acc_finalize_kernel<<<(cells + 255) / 256, 256, 0, st>>>(T64, T, cells, add ? 1 : 0);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+// Which index routine a launch uses: the polynomial path of the configured Doppler source when the host found
+// its error bounds covered by the guard band, else the canonical sequence everywhere.
+int acc_index_mode(const AccParams& p) {
+  if (!p.index_path) return kIdxCanonical;
+  if (p.doppler_mode == SIM_DOPPLER_PULSE_PAIR) return p.pp_ok ? kIdxFastPulsePair : kIdxCanonical;
+  return p.fast_ok ? kIdxFast : kIdxCanonical;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Launchers
 // ---------------------------------------------------------------------------------------------
-size_t acc_tile_smem_bytes(int G, int W, int per_thread) {
-  return (size_t)2 * 7 * kAccThreads * per_thread * sizeof(float) + (size_t)G * W * sizeof(int2);
-}
+typedef void (*AccKernel)(AccParams);
 
-typedef void (*TileKernel)(AccParams);
-
-// (scatterers per thread, resident blocks per SM the register budget is compiled for, index path)
-static TileKernel tile_kernel(int per_thread, int min_blocks, bool fast) {
-  if (per_thread == 2) {
-    if (min_blocks >= 4) return fast ? acc_tile_kernel<2, 4, true> : acc_tile_kernel<2, 4, false>;
-    return fast ? acc_tile_kernel<2, 3, true> : acc_tile_kernel<2, 3, false>;
+static AccKernel acc_kernel_ptr(int ncw, int pt, int il, int mode, bool dbg) {
+#define ACC_CASE(NCW_, PT_, IL_)                                                                       \
+  if (ncw == NCW_ && pt == PT_ && il == IL_) {                                                         \
+    if (dbg)                                                                                           \
+      return mode == kIdxFast ? acc_kernel<NCW_, PT_, IL_, kIdxFast, true>                             \
+           : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, true>           \
+                                       : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, true>;              \
+    return mode == kIdxFast ? acc_kernel<NCW_, PT_, IL_, kIdxFast, false>                              \
+         : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, false>            \
+                                     : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, false>;               \
   }
-  if (min_blocks >= 3) return fast ? acc_tile_kernel<4, 3, true> : acc_tile_kernel<4, 3, false>;
-  return fast ? acc_tile_kernel<4, 2, true> : acc_tile_kernel<4, 2, false>;
+  ACC_CASE(8, 4, 4) ACC_CASE(8, 2, 2) ACC_CASE(16, 4, 4)
+#undef ACC_CASE
+  return nullptr;
 }
 
-cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks) {
-  const size_t smem = acc_tile_smem_bytes(G, W, per_thread);
-  int b = 0;
+bool acc_supported(int ncw, int pt, int il) { return acc_kernel_ptr(ncw, pt, il, kIdxFast, false) != nullptr; }
+
+cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks) {
+  const size_t smem = acc_smem_bytes(G, W, ncw, pt, stages);
   *blocks = 1 << 30;
-  for (int fast = 0; fast < 2; ++fast) {
-    TileKernel k = tile_kernel(per_thread, min_blocks, fast != 0);
+  for (int mode = 0; mode < 3; ++mode) {
+    AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, false);
+    if (!k) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k, kAccThreads, smem);
+    int b = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k, ncw * 32, smem);
     if (e != cudaSuccess) return e;
     if (b < *blocks) *blocks = b;
   }
   return cudaSuccess;
 }
 
-cudaError_t launch_accumulate(const AccParams& p, int variant, int per_thread, int min_blocks, int blocks,
-                              cudaStream_t st, int* launches) {
+// dbg: the same kernel writes (g0, k) per scatterer into p.dbg_g0 / p.dbg_k instead of accumulating.
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  if (variant == 0) {
-    unsigned long long want = (p.n + 255) / 256;
-    const unsigned long long cap = (unsigned long long)blocks * 8;
-    const int grid = (int)(want < cap ? want : cap);
-    acc_reference_kernel<<<grid, 256, 0, st>>>(p);
-    ++*launches;
-    return cudaGetLastError();
-  }
-  const size_t smem = acc_tile_smem_bytes(p.G, p.W, per_thread);
-  cudaError_t e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
+  const int mode = acc_index_mode(p);
+  AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, dbg);
+  if (!k) return cudaErrorInvalidValue;
+  const size_t smem = acc_smem_bytes(p.G, p.W, ncw, pt, p.stages);
+  // per launch: the limit is per function and per device, another handle may have set it for a smaller shape
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
   if (e != cudaSuccess) return e;
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
   const int grid = (int)(n_sc < (unsigned long long)blocks ? n_sc : (unsigned long long)blocks);
-  tile_kernel(per_thread, min_blocks, p.index_path && p.fast_ok)<<<grid, kAccThreads, smem, st>>>(p);
+  k<<<grid, ncw * 32, smem, st>>>(p);
   ++*launches;
   return cudaGetLastError();
 }
 
-cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches) {
+cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  unsigned long long want = (p.n + 255) / 256;
-  const int grid = (int)(want < 148ull * 16 ? want : 148ull * 16);
-  indices_kernel<<<grid, 256, 0, st>>>(p, g0, k);
+  const unsigned long long want = (p.n + 255) / 256;
+  const unsigned long long cap = (unsigned long long)sm_count * 16;
+  acc_reference_kernel<<<(int)(want < cap ? want : cap), 256, 0, st>>>(p);
   ++*launches;
   return cudaGetLastError();
 }

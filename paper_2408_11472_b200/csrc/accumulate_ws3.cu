@@ -411,11 +411,7 @@ __global__ void __launch_bounds__((NCW + 2) * 32, (NCW <= 4 ? 3 : NCW <= 14 ? 2 
 
 // Which index routine a launch uses: the polynomial path of the configured Doppler source when the host found
 // its error bounds covered by the guard band, else the canonical sequence everywhere.
-static int acc_index_mode(const AccParams& p) {
-  if (!p.index_path) return kIdxCanonical;
-  if (p.doppler_mode == SIM_DOPPLER_PULSE_PAIR) return p.pp_ok ? kIdxFastPulsePair : kIdxCanonical;
-  return p.fast_ok ? kIdxFast : kIdxCanonical;
-}
+int acc_index_mode(const AccParams& p);   // accumulate.cu
 
 // ---------------------------------------------------------------------------------------------
 // Index-only kernel (parity pin P11, sim_debug_indices): the index routine of the production kernel
@@ -436,10 +432,10 @@ __global__ void __launch_bounds__(256) indices3_kernel(AccParams p, int32_t* __r
   if (fb) atomicAdd(&p.counters[kCtrFallback], fb);
 }
 
-cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches) {
+cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, int sm_count, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
-  const unsigned long long want = (p.n + 255) / 256;
-  const int grid = (int)(want < 148ull * 16 ? want : 148ull * 16);
+  const unsigned long long want = (p.n + 255) / 256, cap = (unsigned long long)sm_count * 16;
+  const int grid = (int)(want < cap ? want : cap);
   switch (acc_index_mode(p)) {
     case kIdxFast: indices3_kernel<kIdxFast><<<grid, 256, 0, st>>>(p, g0, k); break;
     case kIdxFastPulsePair: indices3_kernel<kIdxFastPulsePair><<<grid, 256, 0, st>>>(p, g0, k); break;
@@ -487,16 +483,13 @@ cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, i
   if (p.n == 0) return cudaSuccess;
   const int mode = acc_index_mode(p);
   // the canonical-everywhere path calls the out-of-line sequence once per scatterer: two in flight per lane are enough
-  const bool swapped = mode == kIdxCanonical && il == 4 && ws3_kernel(ncw, pt, 2, mode);
-  if (swapped) il = 2;
+  if (mode == kIdxCanonical && il == 4 && ws3_kernel(ncw, pt, 2, mode)) il = 2;
   W3Kernel k = ws3_kernel(ncw, pt, il, mode);
   if (!k) return cudaErrorInvalidValue;
   const size_t smem = acc_ws3_smem_bytes(p.G, p.W, ncw, pt, p.stages);
-  cudaError_t e = cudaSuccess;
-  if (swapped) {   // the plan set the shared-memory limit of the planned shape only
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-  }
+  // per launch: the limit is per function and per device, another handle may have set it for a smaller shape
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
   e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
   if (e != cudaSuccess) return e;
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;

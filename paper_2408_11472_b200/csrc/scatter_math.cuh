@@ -2,6 +2,8 @@
 // complex amplitude.  Paper: `scatterers_range`, `scatterers_complex_amplitudes`, the coordinates of
 // `rasterize`.  Used by every accumulation kernel and by the index-only kernel.
 #pragma once
+#include <climits>
+
 #include "sim_internal.h"
 
 namespace simk {
@@ -19,7 +21,7 @@ enum { kIdxCanonical = 0, kIdxFast = 1, kIdxFastPulsePair = 2 };
 // What the index part of one scatterer yields.
 struct Idx {
   int g0;      // gate of the lower half, in [-1, G-1]
-  int k;       // Doppler bin; congruent to the bin mod N (not yet wrapped on the fast path)
+  int k;       // Doppler bin, UNWRAPPED: congruent to the bin mod N, |k| < 2^30
   float w1;    // weight of gate g0+1 (gate g0 gets 1 - w1)
   float fr;    // frac(2R/lambda) mapped to [-0.5, 0.5) cycles
   float gfx;   // gf * 2^kFracBits as a float (for 1/R^2)
@@ -35,7 +37,7 @@ __device__ __forceinline__ float cycles_fraction(double q) {
 // CANONICAL fp64 INDEX SEQUENCE of DESIGN.md, from dx, dy, dz.  Explicit round-to-nearest
 // intrinsics: nvcc must not contract a*b+c differently from the definition.  Out of line (the fast
 // path calls it only inside the guard band) and fed by value.
-// Returns (g0, k wrapped, bits of w1, bits of fr); g0 = SIM_GATE_NONE when the scatterer is dropped.
+// Returns (g0, k unwrapped, bits of w1, bits of fr); g0 = SIM_GATE_NONE when the scatterer is dropped.
 // ---------------------------------------------------------------------------------------------
 struct CanonConsts {
   double rg0, inv_dR, cD, two_over_lambda, fr0, svx, svy, svz, pri, cP;
@@ -66,9 +68,9 @@ static __device__ __noinline__ int4 canonical_tail(CanonConsts c, double dx, dou
   }
   if (!(fabs(kf) < 1073741824.0)) return dropped;
   const double kk = floor(__dadd_rn(kf, 0.5));
-  // N is a power of two: two's-complement AND is the mathematical mod
+  // the bin is returned UNWRAPPED (|kk| < 2^30), like the polynomial path's: whoever needs the bin takes it mod N
   const double q = __fma_rn(delta, c.two_over_lambda, c.fr0);  // only the fraction of 2R/lambda matters
-  return make_int4((int)g0d, ((int)kk) & (c.N - 1), __float_as_int((float)__dsub_rn(gf, g0d)),
+  return make_int4((int)g0d, (int)kk, __float_as_int((float)__dsub_rn(gf, g0d)),
                    __float_as_int(cycles_fraction(q)));
 }
 
@@ -149,6 +151,53 @@ __device__ __forceinline__ bool index_fast(const AccParams& p, const Pre& q, flo
   o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
   o.gfx = (float)gfx;
   return live;
+}
+
+// The same polynomial path in the form the production kernel keeps alive across the amplitude code: the two fixed-point
+// coordinates and the phase; gate, bin, weight and the guard-band test are derived from them afterwards.
+struct Fx {
+  int gfx;     // floor(gf * 2^kFracBits)
+  int kfx;     // floor((kf + 0.5) * 2^kFracBits); INT_MIN when |kf| >= 1024 (the fixed-point read would be meaningless)
+  float fr;    // frac(2R/lambda) mapped to [-0.5, 0.5) cycles
+};
+
+template <int MODE>
+__device__ __forceinline__ Fx index_fx(const AccParams& p, const Pre& q, float xf, float yf, float zf, float vxf, float vyf,
+                                       float vzf) {
+  Fx o;
+  const double u = q.u;
+  const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
+  o.gfx = __double2loint(__dadd_rd(gf, kMagicFx));
+  const double dvx = (double)vxf - p.svx, dvy = (double)vyf - p.svy, dvz = (double)vzf - p.svz;
+  const double num = fma(dvz, q.dz, fma(dvy, q.dy, dvx * q.dx));
+  double kf;
+  if (MODE == kIdxFastPulsePair) {
+    const double dv2 = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
+    const double w = p.pri * fma(dv2, p.pri, num + num);
+    const double e = fma(w, p.inv_2rg0, gf * p.two_dR) * p.inv_2rg0;
+    kf = (w * p.cP_2rg0) * fma(e, e - 1.0, 1.0);
+  } else {
+    kf = num * fma(u, fma(u, p.j2, p.j1), p.j0);
+  }
+  const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));
+  o.kfx = (fabs(kf) < 1024.0) ? kfx : INT_MIN;
+  o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
+  return o;
+}
+
+template <int MODE>
+__device__ __forceinline__ int fx_bin(const AccParams& p, const Fx& f) {
+  return f.kfx >> kFracBits;
+}
+
+// True when a coordinate lies inside the guard band (or the Doppler coordinate was out of the fixed-point range): the
+// canonical sequence has to decide.
+template <int MODE>
+__device__ __forceinline__ bool fx_near(const AccParams& p, const Fx& f) {
+  const int gk = MODE == kIdxFastPulsePair ? p.guard_k : p.guard;   // pulse-pair: wider Doppler guard band
+  const unsigned span = (unsigned)(kFxOne - 2 * p.guard), span_k = (unsigned)(kFxOne - 2 * gk);
+  const int gfrac = f.gfx & (kFxOne - 1), kfrac = f.kfx & (kFxOne - 1);
+  return ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) | (f.kfx == INT_MIN);
 }
 
 // Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.

@@ -18,7 +18,7 @@ thread_local std::string g_create_error;
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  size_t ring_off, slot_bytes, tw_off, ctr_off, stage_off, stage_buf_bytes, iq_off, iq_bytes, total;
+  size_t ring_off, slot_bytes, t64_off, t64_bytes, tw_off, ctr_off, stage_off, stage_buf_bytes, iq_off, iq_bytes, total;
 };
 
 Layout make_layout(const sim_config& c) {
@@ -27,6 +27,9 @@ Layout make_layout(const sim_config& c) {
   L.ring_off = off;
   L.slot_bytes = align_up((size_t)c.n_gates * c.n_doppler * sizeof(float2), 256);
   off += L.slot_bytes * (size_t)c.max_pending_updates;
+  L.t64_off = off;
+  L.t64_bytes = align_up((size_t)c.n_gates * c.n_doppler * sizeof(double2), 256);
+  off += L.t64_bytes;
   L.tw_off = off;
   off += align_up((size_t)(c.n_doppler / 2) * sizeof(float2), 256);
   L.ctr_off = off;
@@ -78,14 +81,13 @@ struct sim_handle {
   int64_t n_updates;             // spectra started so far
   int64_t pulses_emitted;
   // tuning
-  int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard, opt_per_thread, opt_min_blocks;
+  int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard;
   int64_t opt_superchunk;
-  int tile_W, tile_blocks_per_sm;   // cached shared-memory tile geometry (0 = not chosen yet)
-  int opt_ncw, opt_stages;          // warp-specialised kernel: compute warps per block, TMA ring depth (0 = auto)
-  int ws_W, ws_stages, ws_blocks_per_sm;
+  int opt_ncw, opt_stages;          // compute warps per block, TMA ring depth (0 = auto)
+  int ws_W, ws_stages, ws_blocks_per_sm;   // planned window width, ring depth, resident blocks per SM
   int opt_wait_hint, opt_scatter;
   int opt_il;
-  int opt_pt, opt_epoch;            // v3: scatterers per lane per chunk; scatterers per fixed-point epoch (<= 2047)
+  int opt_pt, opt_epoch;            // scatterers per lane per chunk; scatterers per fixed-point epoch
   size_t smem_per_sm;
   // stats
   uint64_t launches, scatterers_seen;
@@ -133,20 +135,6 @@ int check_sat(sim_handle* h, const sim_sat_state* sat) {
   return SIM_OK;
 }
 
-// Shared-memory tile: W Doppler bins x G gates of int2, next to the two input stages.  Small enough for
-// several blocks per SM.
-int choose_window(const sim_handle* h) {
-  const int G = h->cfg.n_gates, N = h->cfg.n_doppler;
-  int w = h->opt_window > 0 ? h->opt_window : 16;
-  if (w > N) w = N;
-  while (w & (w - 1)) w &= w - 1;   // this kernel needs a power of two
-  // default: at most 32 KB of tile next to the stages; an explicit window may use all of shared memory
-  const size_t stages = acc_tile_smem_bytes(0, 0, h->opt_per_thread);
-  const size_t budget = h->opt_window > 0 ? (h->smem_optin > 8192 ? h->smem_optin - 4096 : 4096) : stages + 32 * 1024;
-  while (w > 1 && acc_tile_smem_bytes(G, w, h->opt_per_thread) > budget) w >>= 1;
-  return w;
-}
-
 // Constants of the sqrt/divide-free index path and the decision whether it is valid for this geometry
 // (error bounds that the guard band must cover).
 void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParams& p) {
@@ -165,25 +153,10 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
   const double d_lo = -dR - margin, d_hi = G * dR + margin;
   const double dmax = std::fmax(-d_lo, d_hi), emax = dmax / rg0, rmax = rg0 + d_hi;
   if (!(rg0 + d_lo > 0) || !(emax < 1.0 / 1024.0)) return;
-  p.rg0sq_hi = rg0 * rg0;
-  p.rg0sq_lo = std::fma(rg0, rg0, -p.rg0sq_hi);
-  p.u_lo = d_lo * (2.0 * rg0 + d_lo);
-  p.u_hi = d_hi * (2.0 * rg0 + d_hi);
   p.inv_2rg0 = 0.5 / rg0;
-  p.b1 = -0.5 / rg0;
-  p.b2 = 0.5 / (rg0 * rg0);
-  p.b3 = -0.625 / (rg0 * rg0 * rg0);
-  p.inv_rg0 = 1.0 / rg0;
   const double c = 2.0 / lam;
-  // gate: |delta_fast - delta_canonical| <= sqrt rounding + series truncation + Horner rounding
-  const double err_m = 3e-16 * rmax + 0.06 * std::pow(2.0 * emax, 4) * dmax + 1e-15 * dmax;
-  const double guard_m = p.guard * dR / (double)(1 << kFracBits);
-  // Doppler (|kf| < 1024 on the fast path): 1/R series truncation e^4 + roundings
-  const double err_k = 1024.0 * (std::pow(emax, 4) + 2e-15);
-  const double guard_k = p.guard / (double)(1 << kFracBits);
   const bool phase_ok = (G + 2) * dR * c < 134217728.0;   // 2^27: the magic-number fraction needs |q| < 2^28
-  if (guard_m >= 4.0 * err_m && guard_k >= 4.0 * err_k && phase_ok && G + 2 < 2048) p.fast_ok = 1;
-  {  // polynomial index path of the warp-specialised kernel (scatter_math.cuh), x = u / rg0^2 <= ~2 emax
+  {  // polynomial index path (scatter_math.cuh), x = u / rg0^2 <= ~2 emax
     const double r2 = rg0 * rg0, gd = p.guard / (double)(1 << kFracBits);
     p.neg_rg0sq = -r2;
     p.g1 = 1.0 / (2.0 * rg0 * dR);
@@ -200,9 +173,9 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
     const double x = 2.2 * emax;
     const double eg = 0.04 * x * x * x * x * rg0 / dR + 4.0 * std::ldexp(r2, -52) / (2.0 * rg0 * dR) + 1e-13 * (G + 2);
     const double ek = 1024.0 * (0.32 * x * x * x + 1e-14);
-    if (!(gd >= 4.0 * eg && gd >= 4.0 * ek && phase_ok && G + 2 < 2048)) p.fast_ok = 0;
+    if (gd >= 4.0 * eg && gd >= 4.0 * ek && phase_ok && G + 2 < 2048) p.fast_ok = 1;
   }
-  {  // pulse-pair fast path (scatter_math.cuh, kIdxFastPulsePair).  The canonical R' - R carries the rounding of
+  {  // pulse-pair polynomial path (scatter_math.cuh, kIdxFastPulsePair).  The canonical R' - R carries the rounding of
      // two square roots of ~rmax (each within 2 ulp of the exact root): up to 4 * 2^-53 * rmax * 2N / lambda bins of
      // noise that the (accurate) fast value does not share; the Doppler guard band is 1.5 x that bound.  Series and
      // roundings of the fast value itself: 1024 * (e^3 + 1e-14), e <= 2.2 emax.
@@ -218,76 +191,57 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
     p.pp_ok = (p.fast_ok && gk <= (1 << (kFracBits - 3))) ? 1 : 0;   // the gate half of the bound is the analytic one
     p.guard_k = h->cfg.doppler_mode == SIM_DOPPLER_PULSE_PAIR ? gk : p.guard;
   }
-  // fp32 pre-test: |u_f32 - u| <= 2^-21 R^2 (three squares, two sums, the split satellite position and
-  // rg0^2 each rounded to 2^-24); the margin is twice that at the far edge of the window
-  const double margin_u = std::ldexp(rmax * rmax, -20);
-  p.rg0sq_f = (float)(rg0 * rg0);
-  p.uf_lo = (float)(p.u_lo - margin_u);
-  p.uf_hi = (float)(p.u_hi + margin_u);
 }
 
 int acc_blocks(const sim_handle* h) {
   if (h->opt_blocks > 0) return h->opt_blocks;
-  const int per_sm = h->opt_variant >= 2 ? h->ws_blocks_per_sm : h->tile_blocks_per_sm;
-  return h->sm_count * (per_sm > 0 ? per_sm : 1);
+  return h->sm_count * (h->ws_blocks_per_sm > 0 ? h->ws_blocks_per_sm : 1);
 }
 
-// (Re)chooses the window width and the resident blocks per SM; cheap, called when an option changes.
-cudaError_t plan_tile(sim_handle* h) {
-  h->tile_W = choose_window(h);
-  int b = 1;
-  cudaError_t e = acc_tile_blocks_per_sm(h->cfg.n_gates, h->tile_W, h->opt_per_thread, h->opt_min_blocks, &b);
-  h->tile_blocks_per_sm = b > 0 ? b : 1;
-  return e;
-}
-
-// Per-variant defaults of the warp-specialised kernels (measured on the 268M config, profiles/).
+// Per-variant defaults (measured on the 268M and 16.8M configs, profiles/).
 void variant_defaults(sim_handle* h) {
-  if (h->opt_variant == 3) {
-    h->opt_ncw = 8; h->opt_pt = 4; h->opt_il = 4; h->opt_epoch = 8191;
-  } else {
-    h->opt_ncw = 14; h->opt_pt = 2; h->opt_il = 2; h->opt_epoch = 2047;
-  }
+  h->opt_ncw = 8; h->opt_pt = 4; h->opt_il = 4; h->opt_epoch = 8191;
 }
 
-// Warp-specialised kernel: window width, ring depth and resident blocks per SM for the shared memory there is.
+// Window width, ring depth and resident blocks per SM of the tile kernels for the shared memory there is.
 cudaError_t plan_ws(sim_handle* h) {
+  if (h->opt_variant == 0) {   // the reference kernel has no tile
+    h->ws_W = 1; h->ws_stages = 2; h->ws_blocks_per_sm = 8;
+    return cudaSuccess;
+  }
   const int G = h->cfg.n_gates, N = h->cfg.n_doppler, ncw = h->opt_ncw, pt = h->opt_pt;
   const bool v3 = h->opt_variant == 3;
-  if (v3 && !acc_ws3_supported(ncw, pt, h->opt_il)) return cudaErrorInvalidValue;
-  if (!v3 && ncw != 7 && ncw != 14 && ncw != 22 && ncw != 30) return cudaErrorInvalidValue;
-  auto smem = [&](int g, int w, int st) { return v3 ? acc_ws3_smem_bytes(g, w, ncw, pt, st) : acc_ws_smem_bytes(g, w, ncw, st); };
-  const int target = v3 ? (ncw <= 4 ? 3 : ncw <= 14 ? 2 : 1) : ncw <= 7 ? 4 : (ncw <= 14 ? 2 : 1);   // blocks per SM the register budget allows
+  if (v3 ? !acc_ws3_supported(ncw, pt, h->opt_il) : !acc_supported(ncw, pt, h->opt_il)) return cudaErrorInvalidValue;
+  auto smem = [&](int g, int w, int st) { return v3 ? acc_ws3_smem_bytes(g, w, ncw, pt, st) : acc_smem_bytes(g, w, ncw, pt, st); };
+  const int target = ncw <= 8 ? 2 : 1;                              // blocks per SM the register budget allows
   size_t budget = h->smem_per_sm / target;
   budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
   if (budget > h->smem_optin - 1024) budget = h->smem_optin - 1024;
-  const size_t stage = smem(0, 0, 1);
+  const size_t stage = smem(0, 0, 1) - smem(0, 0, 0);
   int w = h->opt_window > 0 ? h->opt_window : 16;
   if (w > N) w = N;
-  if (!v3) while (w & (w - 1)) w &= w - 1;   // variant 2 needs a power of two
-  while (w > 1 && smem(G, w, 2) > budget) w = v3 ? w - 1 : w >> 1;   // v3 takes any width
-  size_t tiles = smem(G, w, 0);
-  int st = tiles + 2 * stage <= budget ? (int)((budget - tiles) / stage) : 2;
-  if (v3 && h->opt_window == 0 && st < 3) {
-    // a third stage is worth more than the last bins of the window (measured: 16 bins x 2 stages 1.42 ms,
-    // 12 bins x 3 stages 1.39 ms on the 268M config; below 12 bins the escapes take over)
+  auto tiles_of = [&](int ww) { return smem(G, ww, 0); };
+  while (w > 1 && tiles_of(w) + 2 * stage > budget) --w;
+  int st = tiles_of(w) + 2 * stage <= budget ? (int)((budget - tiles_of(w)) / stage) : 2;
+  if (h->opt_window == 0 && st < 3) {
+    // a third stage is worth more than the last bins of the window (measured on the 268M config; below 12 bins the
+    // escapes take over)
     for (int w2 = w - 1; w2 >= 12 && w2 >= 3 * w / 4; --w2) {
-      if (smem(G, w2, 0) + 3 * stage <= budget) {
+      if (tiles_of(w2) + 3 * stage <= budget) {
         w = w2;
-        tiles = smem(G, w, 0);
         st = 3;
         break;
       }
     }
   }
-  const int st_max = v3 ? 6 : 4;
+  const int st_max = v3 ? 6 : 8;
   if (st > st_max) st = st_max;
   if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
   if (st < 2) st = 2;
   h->ws_W = w;
   h->ws_stages = st;
   int b = 1;
-  cudaError_t e = v3 ? acc_ws3_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b) : acc_ws_blocks_per_sm(G, w, ncw, st, &b);
+  cudaError_t e = v3 ? acc_ws3_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b) : acc_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b);
   h->ws_blocks_per_sm = b > 0 ? b : 1;
   return e;
 }
@@ -309,17 +263,10 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   fast_path_constants(h, sat, p);
   const double bn = std::sqrt(sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] +
                               sat->boresight[2] * sat->boresight[2]);
-  p.bx = (float)(sat->boresight[0] / bn);
-  p.by = (float)(sat->boresight[1] / bn);
-  p.bz = (float)(sat->boresight[2] / bn);
-  p.sxh = (float)sat->pos[0]; p.sxl = (float)(sat->pos[0] - (double)p.sxh);
-  p.syh = (float)sat->pos[1]; p.syl = (float)(sat->pos[1] - (double)p.syh);
+  p.sxh = (float)sat->pos[0];
+  p.syh = (float)sat->pos[1];
   p.szh = (float)sat->pos[2]; p.szl = (float)(sat->pos[2] - (double)p.szh);
   p.neg_alpha_log2e = (float)(-h->cfg.antenna_alpha * 1.4426950408889634);
-  p.dR_fx = (float)(h->cfg.gate_spacing_m / (double)(1 << kFracBits));
-  p.dR_f = (float)h->cfg.gate_spacing_m;
-  p.inv_rg0_f = (float)(1.0 / sat->range_gate0_m);
-  p.inv_rg0sq_f = (float)(1.0 / (sat->range_gate0_m * sat->range_gate0_m));
   {  // orthonormal basis (e1, e2) of the plane normal to the boresight: sin^2 = ((d.e1)^2 + (d.e2)^2) / R^2
     const double b[3] = {sat->boresight[0] / bn, sat->boresight[1] / bn, sat->boresight[2] / bn};
     int ax = 0;
@@ -342,38 +289,35 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.G = h->cfg.n_gates;
   p.N = h->cfg.n_doppler;
   p.T = T;
+  p.T64 = reinterpret_cast<double2*>(h->ws + h->lay.t64_off);
   p.counters = counters(h);
-  p.W = h->tile_W;
   const int blocks = acc_blocks(h);
+  const int ch = h->opt_variant == 3 ? acc_ws3_chunk(h->opt_ncw, h->opt_pt) : acc_chunk(h->opt_ncw, h->opt_pt);
   unsigned long long sc = (unsigned long long)h->opt_superchunk;
   if (sc == 0) {
-    // aim at >= 8 scheduling units per block, between one chunk and 64K (v3: 16K) scatterers
-    sc = h->opt_variant == 3 ? 16384 : 65536;
-    while (sc > (unsigned long long)kAccChunk && s->n / sc < (unsigned long long)blocks * 8) sc >>= 1;
+    // aim at >= 8 scheduling units per block, between one chunk and 16K scatterers
+    sc = 16384;
+    while (sc > (unsigned long long)ch && s->n / sc < (unsigned long long)blocks * 8) sc >>= 1;
   }
-  unsigned long long unit = kAccChunk;
-  if (h->opt_variant >= 2) {
-    const int ch = h->opt_variant == 3 ? acc_ws3_chunk(h->opt_ncw, h->opt_pt) : acc_ws_chunk(h->opt_ncw);
-    // chunks per fixed-point epoch: as many as the epoch length allows, but a small input is cut into enough
-    // scheduling units (whole epochs) to give every resident block some work
-    int ec = h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1;
-    if (h->opt_variant == 3) {
-      const unsigned long long fair = s->n / ((unsigned long long)ch * (unsigned long long)blocks * 2ull);
-      if (fair < (unsigned long long)ec) ec = fair > 0 ? (int)fair : 1;
-    }
-    p.W = h->ws_W;
-    p.stages = h->ws_stages;
-    p.wait_hint = (unsigned)h->opt_wait_hint;
-    {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
-      const int L = ec * ch;
-      int lg = 0;
-      while ((1 << lg) < L + 1) ++lg;
-      p.fx_cap = 31 - lg;
-      p.fx_target = p.fx_cap - 2 < 16 ? p.fx_cap - 2 : 16;
-    }
-    p.epoch_chunks = ec;
-    unit = (unsigned long long)ch * p.epoch_chunks;     // super-chunk = whole epochs: a jump never splits one
+  // chunks per fixed-point epoch: as many as the epoch length allows, but a small input is cut into enough
+  // scheduling units (whole epochs) to give every resident block some work
+  int ec = h->opt_epoch / ch > 0 ? h->opt_epoch / ch : 1;
+  {
+    const unsigned long long fair = s->n / ((unsigned long long)ch * (unsigned long long)blocks * 2ull);
+    if (fair < (unsigned long long)ec) ec = fair > 0 ? (int)fair : 1;
   }
+  p.W = h->ws_W;
+  p.stages = h->ws_stages;
+  p.wait_hint = (unsigned)h->opt_wait_hint;
+  {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
+    const int L = ec * ch;
+    int lg = 0;
+    while ((1 << lg) < L + 1) ++lg;
+    p.fx_cap = 31 - lg;
+    p.fx_target = p.fx_cap - 2 < 16 ? p.fx_cap - 2 : 16;
+  }
+  p.epoch_chunks = ec;
+  const unsigned long long unit = (unsigned long long)ch * p.epoch_chunks;   // scheduling unit = whole epochs: a jump never splits one
   sc = (sc + unit - 1) / unit * unit;
   p.superchunk = sc;
   {  // scattered visiting order: dark and illuminated parts of the scene are in flight at the same time, so the
@@ -392,21 +336,46 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   return p;
 }
 
+// The geometry every kernel's fp32 amplitude series is budgeted for (1/R^2 to second order about rg0): window depth
+// <= 0.6 % of rg0 keeps its truncation below 1e-6.
+int check_geometry(sim_handle* h, const sim_sat_state* sat) {
+  const double rg0 = sat->range_gate0_m, depth = (h->cfg.n_gates + 2) * h->cfg.gate_spacing_m;
+  if (!(rg0 > 0)) return fail(h, SIM_ERR_BAD_CONFIG, "range_gate0_m must be > 0");
+  if (!(depth / rg0 <= 6e-3)) return fail(h, SIM_ERR_BAD_CONFIG, "gate window deeper than 0.6 % of range_gate0_m: outside the range of the amplitude series");
+  return SIM_OK;
+}
+
+// One accumulation launch into the fp64 accumulator (variants 0, 4) or straight into T (variant 3).
 int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, float2* T) {
   AccParams p = make_acc_params(h, d_scat, sat, T);
   const int blocks = acc_blocks(h);
   int l = 0;
-  cudaError_t e = h->opt_variant == 3
-                      ? launch_accumulate_ws3(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, h->stream, &l)
-                  : h->opt_variant == 2
-                      ? launch_accumulate_ws(p, h->opt_ncw, blocks, h->stream, &l)
-                      : launch_accumulate(p, h->opt_variant, h->opt_per_thread, h->opt_min_blocks, blocks, h->stream, &l);
+  cudaError_t e = h->opt_variant == 3   ? launch_accumulate_ws3(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, h->stream, &l)
+                  : h->opt_variant == 0 ? launch_reference(p, h->sm_count, h->stream, &l)
+                                        : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
 }
 
-// Common front of the two accumulate entry points: validates, opens a new update if asked.
+// fp64 accumulator -> spectrum slot (assign, or add for SIM_ACC_APPEND); variant 3 has accumulated in place.
+int do_finalize(sim_handle* h, float2* T, bool add) {
+  if (h->opt_variant == 3) return SIM_OK;
+  int l = 0;
+  cudaError_t e = launch_finalize(reinterpret_cast<double2*>(h->ws + h->lay.t64_off), T, h->cfg.n_gates * h->cfg.n_doppler, add,
+                                  h->stream, &l);
+  h->launches += l;
+  if (e != cudaSuccess) return cuda_fail(h, e, "finalize launch");
+  return SIM_OK;
+}
+
+// After a failed launch sequence: whatever reached the fp64 accumulator is discarded (best effort).
+void scrub_accumulator(sim_handle* h) {
+  cudaMemsetAsync(h->ws + h->lay.t64_off, 0, h->lay.t64_bytes, h->stream);
+}
+
+// Common front of the two accumulate entry points: validates everything and says which slot the update uses.
+// Changes NOTHING in the handle: the caller commits (n_updates, scatterers_seen) only after its launches succeeded.
 int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sat, uint32_t flags,
                  bool device_ptrs, float2** T) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
@@ -414,6 +383,8 @@ int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sa
   int rc = check_scatterers(h, s, device_ptrs);
   if (rc) return rc;
   rc = check_sat(h, sat);
+  if (rc) return rc;
+  rc = check_geometry(h, sat);
   if (rc) return rc;
   if (flags & SIM_ACC_APPEND) {
     if (h->n_updates == 0) return fail(h, SIM_ERR_INVALID_ARG, "SIM_ACC_APPEND before any update");
@@ -423,9 +394,6 @@ int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sa
   if (h->n_updates - oldest_needed(h) >= h->cfg.max_pending_updates)
     return fail(h, SIM_ERR_OVERFLOW, "ring full: synthesize pulses before accumulating another update");
   *T = slot_ptr(h, h->n_updates);
-  cudaError_t e = cudaMemsetAsync(*T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
-  if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
-  ++h->n_updates;
   return SIM_OK;
 }
 
@@ -499,10 +467,11 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->ws = static_cast<unsigned char*>(d_workspace);
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->copy_stream = nullptr;
+  h->ev_copied[0] = h->ev_copied[1] = h->ev_consumed[0] = h->ev_consumed[1] = nullptr;
   h->stage_used[0] = h->stage_used[1] = false;
   h->n_updates = 0;
   h->pulses_emitted = 0;
-  h->opt_variant = 3;
+  h->opt_variant = 4;
   variant_defaults(h);
   h->opt_stages = 0;
   h->opt_wait_hint = 0;
@@ -511,33 +480,32 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->opt_window = 0;
   h->opt_index_path = 1;
   h->opt_guard = 16;
-  h->opt_per_thread = 4;
-  h->opt_min_blocks = 3;
-  h->tile_W = 0;
-  h->tile_blocks_per_sm = 0;
   h->opt_superchunk = 0;
+  h->ws_W = 0;
+  h->ws_stages = 0;
+  h->ws_blocks_per_sm = 0;
   h->launches = 0;
   h->scatterers_seen = 0;
   int v = 0;
   e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cfg->device);
-  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)"); }
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)"); }
   h->sm_count = v;
   e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device);
-  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem optin)"); }
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem optin)"); }
   h->smem_optin = (size_t)v;
   if (cfg->host_stage_scatterers > 0 || cfg->host_stage_pulses > 0) {
     e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaStreamCreate(copy)"); }
+    if (e != cudaSuccess) { h->copy_stream = nullptr; sim_destroy(h); return cuda_fail(nullptr, e, "cudaStreamCreate(copy)"); }
     for (int b = 0; b < 2; ++b) {
-      cudaEventCreateWithFlags(&h->ev_copied[b], cudaEventDisableTiming);
-      cudaEventCreateWithFlags(&h->ev_consumed[b], cudaEventDisableTiming);
+      e = cudaEventCreateWithFlags(&h->ev_copied[b], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_consumed[b], cudaEventDisableTiming);
+      if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaEventCreate"); }
     }
   }
   e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, cfg->device);
-  if (e != cudaSuccess) { delete h; return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem per SM)"); }
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem per SM)"); }
   h->smem_per_sm = (size_t)v;
-  e = plan_tile(h);
-  if (e == cudaSuccess) e = plan_ws(h);
+  e = plan_ws(h);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
   {
     int logN = 0;
@@ -546,7 +514,8 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
     if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "synthesis kernel shared-memory attribute"); }
   }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
-  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters)"); }
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->ws + lay.t64_off, 0, lay.t64_bytes, h->stream);
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters, accumulator)"); }
   int l = 0;
   e = launch_twiddles(reinterpret_cast<float2*>(h->ws + lay.tw_off), cfg->n_doppler, h->stream, &l);
   h->launches += l;
@@ -559,8 +528,22 @@ int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim
   float2* T = nullptr;
   int rc = begin_update(h, d_scat, sat, flags, true, &T);
   if (rc) return rc;
+  const bool append = (flags & SIM_ACC_APPEND) != 0;
+  if (h->opt_variant == 3 && !append) {   // variant 3 accumulates straight into the slot
+    cudaError_t e = cudaMemsetAsync(T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
+  }
+  rc = do_accumulate(h, d_scat, sat, T);
+  if (rc == SIM_OK) rc = do_finalize(h, T, append);
+  if (rc) {   // nothing is committed: the update was not started (or, for APPEND, the slot keeps its earlier batches)
+    const std::string msg = h->err;
+    scrub_accumulator(h);
+    h->err = msg;
+    return rc;
+  }
+  if (!append) ++h->n_updates;
   h->scatterers_seen += d_scat->n;
-  return do_accumulate(h, d_scat, sat, T);
+  return SIM_OK;
 }
 
 int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, const sim_sat_state* sat, uint32_t flags) {
@@ -568,42 +551,60 @@ int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, cons
   float2* T = nullptr;
   int rc = begin_update(h, h_scat, sat, flags, false, &T);
   if (rc) return rc;
-  h->scatterers_seen += h_scat->n;
+  const bool append = (flags & SIM_ACC_APPEND) != 0;
+  if (h->opt_variant == 3 && !append) {
+    cudaError_t e = cudaMemsetAsync(T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
+  }
   const uint64_t chunk = (uint64_t)h->cfg.host_stage_scatterers;
   const size_t arr_stride = h->lay.stage_buf_bytes / 7;  // bytes between staged arrays
   const float* src[7] = {h_scat->x, h_scat->y, h_scat->z, h_scat->vx, h_scat->vy, h_scat->vz, h_scat->s0dA};
-  int b = 0;
-  for (uint64_t off = 0; off < h_scat->n; off += chunk, b ^= 1) {
-    const uint64_t m = (h_scat->n - off < chunk) ? h_scat->n - off : chunk;
-    unsigned char* buf = h->ws + h->lay.stage_off + (size_t)b * h->lay.stage_buf_bytes;
-    cudaError_t e;
-    if (h->stage_used[b]) {
-      e = cudaStreamWaitEvent(h->copy_stream, h->ev_consumed[b], 0);  // kernel done with this buffer
-      if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(consumed)");
+  // every chunk is accumulated into the fp64 accumulator; ONE finalize at the end moves the sum into the slot, so a
+  // failure half-way leaves the slot (and the handle) as they were
+  auto run = [&]() -> int {
+    int b = 0;
+    for (uint64_t off = 0; off < h_scat->n; off += chunk, b ^= 1) {
+      const uint64_t m = (h_scat->n - off < chunk) ? h_scat->n - off : chunk;
+      unsigned char* buf = h->ws + h->lay.stage_off + (size_t)b * h->lay.stage_buf_bytes;
+      cudaError_t e;
+      if (h->stage_used[b]) {
+        e = cudaStreamWaitEvent(h->copy_stream, h->ev_consumed[b], 0);  // kernel done with this buffer
+        if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(consumed)");
+      }
+      for (int a = 0; a < 7; ++a) {
+        e = cudaMemcpyAsync(buf + a * arr_stride, src[a] + off, m * sizeof(float), cudaMemcpyHostToDevice, h->copy_stream);
+        if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(H2D scatterers)");
+      }
+      e = cudaEventRecord(h->ev_copied[b], h->copy_stream);
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(copied)");
+      e = cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0);
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(copied)");
+      sim_scatterers d{};
+      d.x = reinterpret_cast<const float*>(buf + 0 * arr_stride);
+      d.y = reinterpret_cast<const float*>(buf + 1 * arr_stride);
+      d.z = reinterpret_cast<const float*>(buf + 2 * arr_stride);
+      d.vx = reinterpret_cast<const float*>(buf + 3 * arr_stride);
+      d.vy = reinterpret_cast<const float*>(buf + 4 * arr_stride);
+      d.vz = reinterpret_cast<const float*>(buf + 5 * arr_stride);
+      d.s0dA = reinterpret_cast<const float*>(buf + 6 * arr_stride);
+      d.n = m;
+      const int rc2 = do_accumulate(h, &d, sat, T);
+      if (rc2) return rc2;
+      e = cudaEventRecord(h->ev_consumed[b], h->stream);
+      if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(consumed)");
+      h->stage_used[b] = true;
     }
-    for (int a = 0; a < 7; ++a) {
-      e = cudaMemcpyAsync(buf + a * arr_stride, src[a] + off, m * sizeof(float), cudaMemcpyHostToDevice, h->copy_stream);
-      if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemcpyAsync(H2D scatterers)");
-    }
-    e = cudaEventRecord(h->ev_copied[b], h->copy_stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(copied)");
-    e = cudaStreamWaitEvent(h->stream, h->ev_copied[b], 0);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamWaitEvent(copied)");
-    sim_scatterers d{};
-    d.x = reinterpret_cast<const float*>(buf + 0 * arr_stride);
-    d.y = reinterpret_cast<const float*>(buf + 1 * arr_stride);
-    d.z = reinterpret_cast<const float*>(buf + 2 * arr_stride);
-    d.vx = reinterpret_cast<const float*>(buf + 3 * arr_stride);
-    d.vy = reinterpret_cast<const float*>(buf + 4 * arr_stride);
-    d.vz = reinterpret_cast<const float*>(buf + 5 * arr_stride);
-    d.s0dA = reinterpret_cast<const float*>(buf + 6 * arr_stride);
-    d.n = m;
-    rc = do_accumulate(h, &d, sat, T);
-    if (rc) return rc;
-    e = cudaEventRecord(h->ev_consumed[b], h->stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaEventRecord(consumed)");
-    h->stage_used[b] = true;
+    return do_finalize(h, T, append);
+  };
+  rc = run();
+  if (rc) {
+    const std::string msg = h->err;
+    scrub_accumulator(h);
+    h->err = msg;
+    return rc;
   }
+  if (!append) ++h->n_updates;
+  h->scatterers_seen += h_scat->n;
   return SIM_OK;
 }
 
@@ -692,8 +693,8 @@ int sim_destroy(sim_handle* h) {
   if (h->copy_stream) {
     cudaStreamSynchronize(h->copy_stream);
     for (int b = 0; b < 2; ++b) {
-      cudaEventDestroy(h->ev_copied[b]);
-      cudaEventDestroy(h->ev_consumed[b]);
+      if (h->ev_copied[b]) cudaEventDestroy(h->ev_copied[b]);
+      if (h->ev_consumed[b]) cudaEventDestroy(h->ev_consumed[b]);
     }
     cudaStreamDestroy(h->copy_stream);
   }
@@ -732,9 +733,12 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   rc = check_sat(h, sat);
   if (rc) return rc;
   AccParams p = make_acc_params(h, &s, sat, nullptr);
+  p.dbg_g0 = d_gate0;
+  p.dbg_k = d_bin;
   int l = 0;
-  cudaError_t e = h->opt_variant >= 2 ? launch_indices3(p, d_gate0, d_bin, h->stream, &l)
-                                      : launch_indices(p, d_gate0, d_bin, h->stream, &l);
+  // the production kernel itself, exporting its indices instead of accumulating (variant 3: its own index kernel)
+  cudaError_t e = h->opt_variant == 3 ? launch_indices3(p, d_gate0, d_bin, h->sm_count, h->stream, &l)
+                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
   return SIM_OK;
@@ -743,17 +747,35 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (value < 0) return fail(h, SIM_ERR_INVALID_ARG, "option value < 0");
+  // options that change the launch shape are re-planned; a shape the kernels do not support restores the old value
+  auto replan = [&](int& field, int v, const char* what) -> int {
+    const int old = field;
+    field = v;
+    const cudaError_t e = plan_ws(h);
+    if (e != cudaSuccess) {
+      field = old;
+      plan_ws(h);
+      cudaGetLastError();
+      return fail(h, SIM_ERR_INVALID_ARG, what);
+    }
+    return SIM_OK;
+  };
   switch (option) {
-    case SIM_OPT_ACC_VARIANT:
-      if (value > 3) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
-      if (value < 2 && h->cfg.doppler_mode == SIM_DOPPLER_PULSE_PAIR)
-        return fail(h, SIM_ERR_INVALID_ARG, "pulse-pair Doppler is implemented by accumulation variants 2 and 3 only");
+    case SIM_OPT_ACC_VARIANT: {
+      if (value != 0 && value != 3 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
+      if (value == 3 && (h->cfg.n_doppler & (h->cfg.n_doppler - 1)))
+        return fail(h, SIM_ERR_INVALID_ARG, "accumulation variant 3 needs a power-of-two n_doppler");
+      const int old = h->opt_variant;
       h->opt_variant = (int)value;
-      variant_defaults(h);   // warps, per-lane count and epoch length are per variant: back to that variant's defaults
-      if (value >= 2) {
-        if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
+      variant_defaults(h);   // warps, per-lane count and epoch length: back to the defaults
+      if (plan_ws(h) != cudaSuccess) {
+        h->opt_variant = old;
+        plan_ws(h);
+        cudaGetLastError();
+        return fail(h, SIM_ERR_INVALID_ARG, "accumulation variant cannot be planned for this configuration");
       }
       return SIM_OK;
+    }
     case SIM_OPT_ACC_BLOCKS:
       if (value > 65535) return fail(h, SIM_ERR_INVALID_ARG, "too many blocks");
       h->opt_blocks = (int)value;
@@ -762,71 +784,39 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       h->opt_superchunk = value;
       return SIM_OK;
     case SIM_OPT_ACC_WINDOW_BINS:
-      if (h->opt_variant != 3 && (value & (value - 1))) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be a power of two (any width with variant 3)");
       if (value > 2048) return fail(h, SIM_ERR_INVALID_ARG, "window bins must be <= 2048");
-      h->opt_window = (int)value;
-      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
-      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
-      return SIM_OK;
-    case SIM_OPT_ACC_PER_THREAD:
-      if (value != 2 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "scatterers per thread must be 2 or 4");
-      h->opt_per_thread = (int)value;
-      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
-      return SIM_OK;
-    case SIM_OPT_ACC_MIN_BLOCKS:
-      if (value < 2 || value > 4) return fail(h, SIM_ERR_INVALID_ARG, "register budget: 2..4 blocks per SM");
-      h->opt_min_blocks = (int)value;
-      if (cudaError_t e = plan_tile(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
-      return SIM_OK;
+      return replan(h->opt_window, (int)value, "window width cannot be planned");
     case SIM_OPT_ACC_WARPS:
-      {
-        const int old = h->opt_ncw;
-        h->opt_ncw = (int)value;
-        if (plan_ws(h) != cudaSuccess) {
-          h->opt_ncw = old;
-          plan_ws(h);
-          return fail(h, SIM_ERR_INVALID_ARG, "compute warps per block not supported by this accumulation variant");
-        }
-      }
-      return SIM_OK;
+      return replan(h->opt_ncw, (int)value, "compute warps per block not supported by this accumulation variant");
     case SIM_OPT_ACC_PER_LANE:
-      {
-        const int old = h->opt_pt;
-        h->opt_pt = (int)value;
-        if (plan_ws(h) != cudaSuccess) {
-          h->opt_pt = old;
-          plan_ws(h);
-          return fail(h, SIM_ERR_INVALID_ARG, "scatterers per lane not supported by this accumulation variant");
-        }
+      return replan(h->opt_pt, (int)value, "scatterers per lane not supported by this accumulation variant");
+    case SIM_OPT_ACC_SHAPE: {
+      const int ncw = (int)(value >> 16), pt = (int)((value >> 8) & 255), il = (int)(value & 255);
+      const int o_ncw = h->opt_ncw, o_pt = h->opt_pt, o_il = h->opt_il;
+      h->opt_ncw = ncw; h->opt_pt = pt; h->opt_il = il;
+      if (plan_ws(h) != cudaSuccess) {
+        h->opt_ncw = o_ncw; h->opt_pt = o_pt; h->opt_il = o_il;
+        plan_ws(h);
+        cudaGetLastError();
+        return fail(h, SIM_ERR_INVALID_ARG, "block shape (warps, per lane, interleave) not compiled for this accumulation variant");
       }
       return SIM_OK;
+    }
     case SIM_OPT_ACC_WAIT_HINT:
       h->opt_wait_hint = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_INTERLEAVE:
-      {
-        const int old = h->opt_il;
-        h->opt_il = (int)value;
-        if (plan_ws(h) != cudaSuccess) {
-          h->opt_il = old;
-          plan_ws(h);
-          return fail(h, SIM_ERR_INVALID_ARG, "interleave not supported by this accumulation variant");
-        }
-      }
-      return SIM_OK;
+      return replan(h->opt_il, (int)value, "interleave not supported by this accumulation variant");
     case SIM_OPT_ACC_SCATTER:
       h->opt_scatter = value != 0;
       return SIM_OK;
     case SIM_OPT_ACC_EPOCH:
-      if (value < 64 || value > 16383 || (h->opt_variant != 3 && value > 2047))
-        return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..2047 (variant 3: ..16383)");
+      if (value < 64 || value > 16383) return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..16383");
       h->opt_epoch = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_STAGES:
-      if (value > 6 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..6 (variant 2: at most 4)");
-      h->opt_stages = (int)value;
-      if (cudaError_t e = plan_ws(h)) return cuda_fail(h, e, "accumulation kernel occupancy query");
-      return SIM_OK;
+      if (value > 8 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..8");
+      return replan(h->opt_stages, (int)value, "ring depth cannot be planned");
     case SIM_OPT_GUARD_LSB:
       if (value < 1 || value > (1 << (kFracBits - 2))) return fail(h, SIM_ERR_INVALID_ARG, "guard must be in 1..2^18");
       h->opt_guard = (int)value;
@@ -853,7 +843,12 @@ int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (!h_out) return fail(h, SIM_ERR_INVALID_ARG, "h_out is NULL");
   cudaError_t e = cudaMemcpyAsync(h_out, counters(h), 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, h->stream);
-  if (e == cudaSuccess && reset) e = cudaMemsetAsync(counters(h), 0, 4 * sizeof(uint32_t), h->stream);
+  if (getenv("SIM_PROFILE")) {
+    unsigned long long pr[5];
+    cudaMemcpy(pr, counters(h) + 8, sizeof(pr), cudaMemcpyDeviceToHost);
+    fprintf(stderr, "PROF wait_full %.3f wait_tile %.3f drain %.3f issue %.3f of total warp-cycles %llu\n", pr[0] / (double)pr[4], pr[1] / (double)pr[4], pr[2] / (double)pr[4], pr[3] / (double)pr[4], pr[4]);
+  }
+  if (e == cudaSuccess && reset) e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(uint32_t), h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "read counters");
   return SIM_OK;

@@ -7,16 +7,13 @@
 
 namespace simk {
 
-constexpr int kAccThreads = 256;              // threads per block of the tile accumulation kernel
-constexpr int kAccWarps = kAccThreads / 32;
-constexpr int kAccChunk = kAccThreads * 4;    // largest chunk (4 scatterers per thread) = one fixed-point epoch
 constexpr int kNumCounters = 64;
 constexpr int kFracBits = 20;                 // fixed-point fraction bits of the gate / Doppler coordinates
 
 enum Counter : int {
   kCtrTicket = 0,   // scheduling ticket of the running accumulation launch
-  kCtrEscape = 1,   // contributions sent to global atomics (outside the window or above the fixed-point range)
-  kCtrFlush = 2,    // unused (the tile drains to global every epoch)
+  kCtrEscape = 1,   // contributions sent to global reductions (guard band, outside the window or the fixed-point range)
+  kCtrUnused = 2,
   kCtrFallback = 3, // scatterers whose indices were decided by the canonical sequence (guard band)
 };
 
@@ -33,53 +30,47 @@ struct AccParams {
   double cD;              // (-2.0 * N) / (wavelength * PRF)
   double pri, cP;         // pulse-pair Doppler: 1.0 / PRF and (-2.0 * N) / wavelength
   int doppler_mode;       // SIM_DOPPLER_*
-  // ---- fast index path: delta = R - rg0 from u = R^2 - rg0^2 by series, no sqrt / div ----
-  double rg0sq_hi, rg0sq_lo;  // rg0^2 as an exact double-double
-  double u_lo, u_hi;          // u outside [u_lo, u_hi] is certainly outside the gate window
-  double inv_2rg0;            // 1 / (2 rg0)
-  double b1, b2, b3;          // delta = t (1 + t (b1 + t (b2 + t b3))),  t = u / (2 rg0)
-  double inv_rg0;             // 1 / rg0
-  double fr0;                 // frac(rg0 * 2 / lambda), exact to ~1e-17
-  int guard;                  // guard band in units of 2^-kFracBits around integer gate / bin boundaries
-  int guard_k;                // the same for the Doppler coordinate (wider for the pulse-pair path)
-  int fast_ok;                // host-side validity of the fast path for this geometry (analytic Doppler)
-  int pp_ok;                  // ... of the pulse-pair fast path
-  double two_dR, cP_2rg0;     // pulse-pair fast path: 2 * gate_spacing, cP / (2 rg0)
-  // ---- fp32 amplitude path ----
-  float sxh, sxl, syh, syl, szh, szl;  // satellite position as float hi + lo
-  float bx, by, bz;                    // unit boresight
-  float neg_alpha_log2e;               // -antenna_alpha * log2(e)
-  float dR_fx;                         // gate_spacing * 2^-kFracBits
-  float dR_f;                          // gate_spacing
-  float inv_rg0_f;                     // 1 / rg0
-  float inv_rg0sq_f;                   // 1 / rg0^2
-  float rg0sq_f, uf_lo, uf_hi;         // fp32 pre-test: u_f32 = R^2 - rg0^2 outside [uf_lo, uf_hi] is certainly out
-  int G, N;
-  float2* T;              // spectrum of the current update, [G][N]
-  unsigned int* counters; // kNumCounters device words
-  unsigned long long superchunk; // scatterers per scheduling unit (multiple of kAccChunk)
-  int W;                  // Doppler bins of the shared-memory window (power of two, <= N)
-  int index_path;         // 0 canonical everywhere, 1 fast path + guard band
-  // ---- warp-specialised kernel (accumulate_ws.cu): polynomial index path in u = R^2 - rg0^2 ----
+  double fr0;             // frac(rg0 * 2 / lambda), exact to ~1e-17
+  // ---- polynomial index path in u = R^2 - rg0^2: no sqrt, no divide ----
+  int index_path;         // 0 canonical everywhere, 1 polynomial path + guard band
+  int guard;              // guard band in units of 2^-kFracBits around integer gate boundaries
+  int guard_k;            // the same for the Doppler coordinate (wider for the pulse-pair path)
+  int fast_ok;            // host-side validity of the polynomial path for this geometry (analytic Doppler)
+  int pp_ok;              // ... of the pulse-pair polynomial path
   double neg_rg0sq;       // -(rg0 * rg0), rounded once
   double uw_lo, uw_hi;    // u outside [uw_lo, uw_hi]: outside the gate window by more than half a guard band
   double g1, g2, g3;      // gf = u (g1 + u (g2 + u g3))            = (R - rg0) / dR
   double j0, j1, j2;      // kf = num (j0 + u (j1 + u j2))          = num cD / R
   double cq;              // dR * 2 / lambda: cycles of phase per gate
+  double inv_2rg0, two_dR, cP_2rg0;   // pulse-pair polynomial path: 1 / (2 rg0), 2 * gate_spacing, cP / (2 rg0)
+  // ---- fp32 amplitude path ----
+  float sxh, syh, szh, szl;            // satellite position as float (z as hi + lo)
+  float neg_alpha_log2e;               // -antenna_alpha * log2(e)
   float e1x, e1y, e1z, e2x, e2y, e2z;  // orthonormal basis of the plane normal to the boresight
   float a0, a1, a2;       // 1/R^2 = a0 + gfx (a1 + gfx a2), gfx = gf * 2^kFracBits
   float w_scale;          // 2^-kFracBits
+  // ---- tabulated antenna gain on a u-v grid (reading R9); lut == nullptr: analytic gain ----
+  const float2* lut;      // [lut_nv][lut_nu] complex gain, u fastest
+  int lut_nu, lut_nv;
+  float lut_u0, lut_v0, lut_inv_du, lut_inv_dv;
+  int G, N;
+  float2* T;              // spectrum of the current update, [G][N] (variant 3 accumulates into it directly)
+  double2* T64;           // fp64 accumulator [G][N] (variants 0, 4): zero between updates, rounded to T by the finalize kernel
+  int32_t *dbg_g0, *dbg_k;   // index export of the production kernel (sim_debug_indices)
+  unsigned int* counters; // kNumCounters device words
+  unsigned long long superchunk; // scatterers per scheduling unit (whole fixed-point epochs)
+  int W;                  // Doppler bins of the shared-memory window
   int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
-  int fx_cap, fx_target;     // v3 block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
-  unsigned long long sc_stride;  // v3: super-chunk visited by ticket t is (t * sc_stride) mod n_superchunks (coprime)
-  unsigned wait_hint;        // v3: suspend-time hint of the mbarrier waits in ns (0 = plain try_wait loop)
+  int fx_cap, fx_target;     // block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
+  unsigned long long sc_stride;  // scheduling unit visited by ticket t is (t * sc_stride) mod n_units (coprime)
+  unsigned wait_hint;        // variant 3: suspend-time hint of the mbarrier waits in ns (0 = plain try_wait loop)
 };
 
 struct SynParams {
   const float2* ring;     // spectra ring base
   size_t slot_stride;     // float2 elements per slot
   int cap;                // ring capacity
-  const float2* tw;       // twiddles exp(+2 pi i j / N), j < N/2
+  const float2* tw;       // twiddles exp(+2 pi i j / N), j < N
   float2* iq;             // output [n_pulses][G]
   long long x0;           // first pulse of this call
   long long n_pulses;
@@ -90,25 +81,21 @@ struct SynParams {
   int weight_mode;
 };
 
-cudaError_t launch_accumulate(const AccParams& p, int variant, int per_thread, int min_blocks, int blocks,
-                              cudaStream_t st, int* launches);
-// warp-specialised kernel: ncw compute warps + 1 control warp per block
-size_t acc_ws_smem_bytes(int G, int W, int ncw, int stages);
-cudaError_t acc_ws_blocks_per_sm(int G, int W, int ncw, int stages, int* blocks);
-cudaError_t launch_accumulate_ws(const AccParams& p, int ncw, int blocks, cudaStream_t st, int* launches);
-int acc_ws_chunk(int ncw);
-// v3: producer warp + drain warp + ncw compute warps, pt scatterers per lane per chunk
+// production kernel (accumulate.cu): ncw compute warps + 1 drain warp per block, pt scatterers per lane per chunk
+int acc_chunk(int ncw, int pt);
+size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages);
+bool acc_supported(int ncw, int pt, int il);
+cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches);
+cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches);
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches);
+// round-1 production kernel, kept for A/B (accumulate_ws3.cu): producer warp + drain warp + ncw compute warps
 size_t acc_ws3_smem_bytes(int G, int W, int ncw, int pt, int stages);
 bool acc_ws3_supported(int ncw, int pt, int il);
 cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
 cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, int blocks, cudaStream_t st, int* launches);
 int acc_ws3_chunk(int ncw, int pt);
-cudaError_t launch_indices(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st,
-                           int* launches);
-// the index routine of the warp-specialised kernels (variants 2 and 3)
-cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, cudaStream_t st, int* launches);
-size_t acc_tile_smem_bytes(int G, int W, int per_thread);
-cudaError_t acc_tile_blocks_per_sm(int G, int W, int per_thread, int min_blocks, int* blocks);
+cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, int sm_count, cudaStream_t st, int* launches);
 // regular mode (regular.cu): Y[n_pulses][G] += per-pulse coherent sums; cudaErrorInvalidConfiguration when G is too
 // large for one pulse row per thread in shared memory
 cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,

@@ -21,8 +21,8 @@ DOPPLER_ANALYTIC, DOPPLER_PULSE_PAIR = 0, 1
 SYN_FINAL = 1
 GATE_NONE = -(2**31)
 OPT_ACC_VARIANT, OPT_ACC_BLOCKS, OPT_ACC_SUPERCHUNK, OPT_ACC_WINDOW_BINS, OPT_GUARD_LSB, OPT_INDEX_PATH = 1, 2, 3, 4, 5, 6
-OPT_ACC_PER_THREAD, OPT_ACC_MIN_BLOCKS, OPT_ACC_WARPS, OPT_ACC_STAGES = 7, 8, 9, 10
-OPT_ACC_PER_LANE, OPT_ACC_EPOCH, OPT_ACC_WAIT_HINT, OPT_ACC_SCATTER, OPT_ACC_INTERLEAVE = 11, 12, 13, 14, 15
+OPT_ACC_WARPS, OPT_ACC_STAGES = 9, 10
+OPT_ACC_PER_LANE, OPT_ACC_EPOCH, OPT_ACC_WAIT_HINT, OPT_ACC_SCATTER, OPT_ACC_INTERLEAVE, OPT_ACC_SHAPE = 11, 12, 13, 14, 15, 16
 
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",

@@ -32,7 +32,7 @@ def _indices_exact(orc, sim_mod, wl, scat_cuda, scat_np, sim, u=0, index_path=No
 
 
 # ---- configs[0]: Tiny, full size, every accumulation variant ----------------------------------------
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 3, 4])
 def test_tiny_full(oracle, sim_mod, variant):
     wl = W.get("tiny")
     scat = W.scatterers(wl)
@@ -65,7 +65,7 @@ def test_reduced_configs(oracle, sim_mod, name):
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
     assert np.abs(T_ref).max() > 0
-    for variant in (0, 1, 2, 3):
+    for variant in (0, 3, 4):
         T, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda, options={sim_mod.OPT_ACC_VARIANT: variant})
         U.check_stream(oracle, wl, T, iq, T_ref)
     for u in (0, wl.n_updates - 1):
@@ -203,7 +203,7 @@ def test_append_equals_single_call_and_linearity(oracle, sim_mod):
 
 # ---- edge cases ------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n", [0, 1, 3, 4, 5, 2047, 2048, 2049, 3 * 2048 + 5])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 3, 4])
 def test_ragged_sizes(oracle, sim_mod, n, variant):
     wl = W.get("tiny").scaled(n_updates=1)
     scat = {k: v[:n].contiguous() for k, v in W.scatterers(wl).items()}
@@ -218,7 +218,7 @@ def test_ragged_sizes(oracle, sim_mod, n, variant):
         _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 3, 4])
 def test_degenerate_inputs(oracle, sim_mod, variant):
     """Out-of-window, dead (s0dA <= 0, NaN), non-finite positions/velocities: dropped on both sides."""
     wl = W.get("tiny").scaled(n_updates=1)
@@ -346,12 +346,12 @@ def test_heavy_tailed_amplitudes(oracle, sim_mod):
     assert U.rel_l2(sim.get_spectrum(1).cpu().numpy(), T_ref) <= U.TOL
 
 
-V3_SHAPES = [(8, 2, 2), (8, 4, 4), (8, 4, 2), (12, 2, 2), (16, 4, 2), (20, 4, 2)]
+ACC_SHAPES = [(8, 2, 2), (8, 4, 4), (16, 4, 4)]
 
 
-@pytest.mark.parametrize("ncw,pt,il", V3_SHAPES)
-def test_v3_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
-    """Production kernel (variant 3): every compiled block shape, short to very long fixed-point epochs (the
+@pytest.mark.parametrize("ncw,pt,il", ACC_SHAPES)
+def test_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
+    """Production kernel (variant 4): every compiled block shape, short to very long fixed-point epochs (the
     admitted magnitude range shrinks as the epoch grows so that no cell can overflow), scattered visiting
     order, tiny scheduling units, on a scene with out-of-window parts and a ragged tail."""
     wl = W.get("sar_footprint_268m").scaled(n_along=509, n_cross=1031, spacing_m=13.0, n_updates=1)
@@ -361,11 +361,7 @@ def test_v3_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
     for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 0}), (4095, {sim_mod.OPT_ACC_STAGES: 2, sim_mod.OPT_ACC_WINDOW_BINS: 11}),
                          (8191, {sim_mod.OPT_ACC_SUPERCHUNK: 1}), (16383, {sim_mod.OPT_ACC_BLOCKS: 3})):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
-        sim.set_option(sim_mod.OPT_ACC_VARIANT, 3)
-        sim.set_option(sim_mod.OPT_ACC_INTERLEAVE, 2)       # each intermediate combination is a compiled shape
-        sim.set_option(sim_mod.OPT_ACC_PER_LANE, pt)
-        sim.set_option(sim_mod.OPT_ACC_WARPS, ncw)
-        sim.set_option(sim_mod.OPT_ACC_INTERLEAVE, il)
+        sim.set_option(sim_mod.OPT_ACC_SHAPE, (ncw << 16) | (pt << 8) | il)
         sim.set_option(sim_mod.OPT_ACC_EPOCH, epoch)
         for k, v in extra.items():
             sim.set_option(k, v)
@@ -389,7 +385,7 @@ def test_coherent_pileup_cannot_overflow(oracle, sim_mod):
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
     assert (np.abs(T_ref) > 0).sum() == 2                       # one bin, two gate halves
-    for variant, epoch in ((2, 2047), (3, 2047), (3, 8191), (3, 16383)):
+    for variant, epoch in ((4, 2047), (4, 8191), (4, 16383)):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
         sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
         sim.set_option(sim_mod.OPT_ACC_EPOCH, epoch)
@@ -418,7 +414,7 @@ def test_pulse_pair_doppler(oracle, sim_mod, name):
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     updates = [0, wl.n_updates - 1]
     pp = oracle.DOPPLER_PULSE_PAIR
-    for variant in (3, 2):
+    for variant in (4, 3, 0):
         sim = sim_mod.Sim(sim_mod.config_for(wl, doppler_mode=sim_mod.DOPPLER_PULSE_PAIR, max_pending_updates=2))
         sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
         for j, u in enumerate(updates):
@@ -436,8 +432,6 @@ def test_pulse_pair_doppler(oracle, sim_mod, name):
     differ = int((ka != kp).sum())
     assert 0 < differ < 0.02 * wl.n_scatterers
     sim = sim_mod.Sim(sim_mod.config_for(wl, doppler_mode=sim_mod.DOPPLER_PULSE_PAIR))
-    with pytest.raises(sim_mod.SimError):
-        sim.set_option(sim_mod.OPT_ACC_VARIANT, 1)                 # variants 0 and 1 do not implement it
     # polynomial path + guard band (default) against the canonical sequence everywhere: same bins, and the
     # guard band stays thin although it is wider than the analytic one (it covers the cancellation noise of R' - R)
     sim.read_counters(reset=True)
@@ -618,10 +612,8 @@ def test_argument_errors(sim_mod):
         sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, 4096)       # wider than the largest N
     with pytest.raises(sim_mod.SimError):
         sim.set_option(sim_mod.OPT_ACC_EPOCH, 1 << 20)          # beyond the overflow-safe epoch length
-    sim.set_option(sim_mod.OPT_ACC_VARIANT, 2)
     with pytest.raises(sim_mod.SimError):
-        sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, 3)          # variants 1 and 2 need a power of two
-    sim.set_option(sim_mod.OPT_ACC_VARIANT, 3)
+        sim.set_option(sim_mod.OPT_ACC_VARIANT, 2)              # the superseded kernels are gone
     assert sim.stats()["updates_accumulated"] == 0   # errors leave the handle unchanged
     sim.accumulate_update(scat, sim_mod.sat_for(wl, 0))
     assert sim.stats()["updates_accumulated"] == 1 and sim.stats()["kernel_launches"] >= 2

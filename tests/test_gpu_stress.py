@@ -1,6 +1,6 @@
 """Randomised (seeded) sweep over scene shapes, sizes, Doppler modes and every tuning knob of the production
 accumulation kernel: each draw must match the oracle (rel L2 <= 1e-4) and, above all, terminate: the kernel's
-producer / compute / drain warps talk through mbarriers only, so a missed arrival would hang, not fail."""
+compute and drain warps talk through mbarriers and shared-memory counters only, so a missed arrival would hang, not fail."""
 import random
 
 import numpy as np
@@ -12,7 +12,7 @@ from tests import gpu_util as U
 
 pytestmark = [pytest.mark.gpu, pytest.mark.timeout(600)]
 
-SHAPES = [(8, 2, 2), (8, 4, 4), (8, 4, 2), (12, 2, 2), (16, 4, 2), (20, 4, 2)]
+SHAPES = [(8, 2, 2), (8, 4, 4), (16, 4, 4)]
 
 
 @pytest.mark.parametrize("seed", [11, 12, 13])
@@ -39,9 +39,9 @@ def test_random_shapes_and_options(oracle, seed):
         dm = rnd.choice([0, 0, 1])
         sim = S.Sim(S.config_for(wl, doppler_mode=dm))
         ncw, pt, il = rnd.choice(SHAPES)
-        opts = [(S.OPT_ACC_INTERLEAVE, 2), (S.OPT_ACC_PER_LANE, pt), (S.OPT_ACC_WARPS, ncw), (S.OPT_ACC_INTERLEAVE, il),
+        opts = [(S.OPT_ACC_SHAPE, (ncw << 16) | (pt << 8) | il),
                 (S.OPT_ACC_EPOCH, rnd.choice([64, 500, 1024, 2047, 8191, 16383])),
-                (S.OPT_ACC_STAGES, rnd.choice([0, 2, 3, 4, 6])),
+                (S.OPT_ACC_STAGES, rnd.choice([0, 2, 3, 4, 8])),
                 (S.OPT_ACC_BLOCKS, rnd.choice([0, 1, 2, 5, 37, 296, 1000])),
                 (S.OPT_ACC_SUPERCHUNK, rnd.choice([0, 1, 4096, 100000])),
                 (S.OPT_ACC_WINDOW_BINS, rnd.choice([0, 1, 3, 7, 12, 16])),
@@ -53,4 +53,4 @@ def test_random_shapes_and_options(oracle, seed):
         T = sim.get_spectrum(0).cpu().numpy()
         T_ref = U.oracle_spectra(oracle, wl, U.to_numpy(scat), [0], doppler_mode=dm, nthreads=4)[0]
         e = U.rel_l2(T, T_ref)
-        assert e <= U.TOL, (seed, trial, e, G, N, n, sea, dm, (ncw, pt, il), opts[4:])
+        assert e <= U.TOL, (seed, trial, e, G, N, n, sea, dm, (ncw, pt, il), opts[1:])
