@@ -88,28 +88,22 @@ __device__ __forceinline__ void publish_unit(const AccParams& p, const UnitTable
   }
 }
 
-// Position of a chunk in the block's sequence: unit index and chunk index inside the unit; advanced chunk by chunk.
-struct ChunkPos {
-  unsigned unit, r;
-  __device__ __forceinline__ void advance(unsigned cps) {
-    if (++r == cps) {
-      r = 0;
-      ++unit;
-    }
-  }
+// A stream of chunks through the block's units (one for the copies, one for the reads): the current unit and the run
+// [base, end) of it that is left, in registers.  The unit table is consulted only when a unit is exhausted.
+struct ChunkStream {
+  unsigned long long base, end;   // next chunk starts at base; base >= end: the unit is exhausted
+  unsigned unit;                  // index of the unit [base, end) belongs to (the next one to open when exhausted)
+  bool stop;                      // the end of work has been seen
 };
 
-// First scatterer and valid count of the chunk at `pos`; returns false at the end of work (an empty unit).  The last unit
-// of the scene may be short: its trailing chunks are empty (count 0) but not the end.  Called by all lanes together.
-template <int CH>
-__device__ __forceinline__ bool chunk_range(const UnitTable& ut, const ChunkPos& pos, unsigned long long& base, unsigned& nvalid) {
-  const unsigned slot = pos.unit & (kRing - 1);
-  while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != pos.unit + 1u) {
+// Opens unit s.unit (waits for its publication, all lanes together).  An empty unit is the end of work.
+__device__ __forceinline__ void stream_open(const UnitTable& ut, ChunkStream& s) {
+  const unsigned slot = s.unit & (kRing - 1);
+  while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != s.unit + 1u) {
   }
-  const unsigned long long start = sh::ld64(ut.start0 + 8u * slot), end = sh::ld64(ut.end0 + 8u * slot);
-  base = start + (unsigned long long)pos.r * CH;
-  nvalid = base < end ? (unsigned)((end - base < (unsigned long long)CH) ? end - base : CH) : 0u;
-  return end != 0ull;
+  s.base = sh::ld64(ut.start0 + 8u * slot);
+  s.end = sh::ld64(ut.end0 + 8u * slot);
+  s.stop = s.end == 0ull;
 }
 
 // round(a * b) for |a b| <= 2^22 by the 1.5 * 2^23 trick (round to nearest even: unbiased), as an int
@@ -185,9 +179,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   const unsigned complete0 = sh::addr(&s_complete[0]), shares0 = sh::addr(&s_shares[0]);
   const unsigned slot0 = sh::addr(&s_slot[0][0]);
   const unsigned cps = (unsigned)(p.superchunk / CH);          // chunks per scheduling unit
-  // the copies run S - 1 chunks ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
+  // the copies run one chunk ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
   // need before the end of the chunk in which it is published
-  const unsigned ahead = ((unsigned)S - 1u + cps - 1u) / cps + 1u;
+  const unsigned ahead = 2u;   // (two stages: the copies are one chunk ahead of the reads, at most one unit ahead)
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
   const unsigned e0 = (unsigned)lane * PT;             // this lane's first scatterer in the warp's slice
   const unsigned slice_lo = (unsigned)warp * SL;       // the warp's slice in a chunk
@@ -214,33 +208,34 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   __syncthreads();
 
   PendingUnit tk{0u, 0u, false};
-  // This lane's PT scatterers of the chunk at `pos` (7 x 16 bytes) -> its place in stage `st`; one commit group per chunk,
-  // empty beyond the end of the input.  PT = 2 lanes pair up: the even lane copies for both.
-  auto copy_chunk = [&](const ChunkPos& pos, unsigned st) {
-    unsigned long long base;
-    unsigned nv;
-    chunk_range<CH>(ut, pos, base, nv);
-    const unsigned n4 = nv & ~3u;
-    const unsigned o4 = (slice_lo + e0) & ~3u;                    // first scatterer of this lane's 16-byte group
-    if ((PT == 4 || !(lane & 1)) && o4 + 4u <= n4) {
-      const unsigned dst = stage0 + st * kStageBytes + o4 * 4u;
-      const unsigned long long g = base + o4;
-      sh::cp_async16(dst + 0u * CH * 4u, p.x + g);
-      sh::cp_async16(dst + 1u * CH * 4u, p.y + g);
-      sh::cp_async16(dst + 2u * CH * 4u, p.z + g);
-      sh::cp_async16(dst + 3u * CH * 4u, p.vx + g);
-      sh::cp_async16(dst + 4u * CH * 4u, p.vy + g);
-      sh::cp_async16(dst + 5u * CH * 4u, p.vz + g);
-      sh::cp_async16(dst + 6u * CH * 4u, p.s0dA + g);
+  // This lane's PT scatterers of the next chunk of the copy stream (7 x 16 bytes) -> its place in stage `st`; one commit
+  // group per chunk, empty beyond the end of the input.  PT = 2 lanes pair up: the even lane copies for both.
+  ChunkStream cs{0ull, 0ull, 0u, false}, rs{0ull, 0ull, 0u, false};
+  auto copy_chunk = [&](unsigned st) {
+    if (cs.base >= cs.end && !cs.stop) {   // (rare) the next unit
+      stream_open(ut, cs);
+      ++cs.unit;
+    }
+    if (!cs.stop) {
+      const unsigned long long left = cs.end - cs.base;
+      const unsigned n4 = left >= (unsigned long long)CH ? (unsigned)CH : ((unsigned)left & ~3u);
+      const unsigned o4 = (slice_lo + e0) & ~3u;                    // first scatterer of this lane's 16-byte group
+      if ((PT == 4 || !(lane & 1)) && o4 + 4u <= n4) {
+        const unsigned dst = stage0 + st * kStageBytes + o4 * 4u;
+        const unsigned long long g = cs.base + o4;
+        sh::cp_async16(dst + 0u * CH * 4u, p.x + g);
+        sh::cp_async16(dst + 1u * CH * 4u, p.y + g);
+        sh::cp_async16(dst + 2u * CH * 4u, p.z + g);
+        sh::cp_async16(dst + 3u * CH * 4u, p.vx + g);
+        sh::cp_async16(dst + 4u * CH * 4u, p.vy + g);
+        sh::cp_async16(dst + 5u * CH * 4u, p.vz + g);
+        sh::cp_async16(dst + 6u * CH * 4u, p.s0dA + g);
+      }
+      cs.base += CH;
     }
     sh::cp_async_commit();
   };
-  ChunkPos cpos{0u, 0u};   // the chunk to copy next
-  ChunkPos rpos{0u, 0u};   // the chunk to read next
-  for (int s = 0; s + 1 < S; ++s) {   // chunks 0 .. S-2 are in flight
-    copy_chunk(cpos, (unsigned)s);
-    cpos.advance(cps);
-  }
+  copy_chunk(0u);   // chunk 0 is in flight (two stages: the copies run one chunk ahead of the reads)
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
@@ -330,36 +325,30 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     float s = 0.0f, sS = 0.0f, sO = 0.0f;
     int ci = 0;
     for (; ci < EC; ++ci) {
-      if (!DBG && dpend < e) try_drain(e, false);
-      // chunk cidx + S - 1 goes into the stage that was read one iteration ago; then this lane's copies of chunk cidx
-      // (S - 1 groups older) must have landed
-      copy_chunk(cpos, stg == 0 ? (unsigned)S - 1u : stg - 1u);
-      cpos.advance(cps);
-      switch (S) {
-        case 2: sh::cp_async_wait<1>(); break;
-        case 3: sh::cp_async_wait<2>(); break;
-        case 4: sh::cp_async_wait<3>(); break;
-        case 5: sh::cp_async_wait<4>(); break;
-        case 6: sh::cp_async_wait<5>(); break;
-        case 7: sh::cp_async_wait<6>(); break;
-        default: sh::cp_async_wait<7>(); break;
-      }
+      if (!DBG && dpend < e && sh::ld_acquire(complete0 + 4u * (dpend & 1u)) > (int)(dpend >> 1)) try_drain(e, false);
+      // the next chunk goes into the stage that was read one iteration ago; then this lane's copies of the chunk to read
+      // (one group older) must have landed
+      copy_chunk(stg ^ 1u);
+      sh::cp_async_wait<1>();
       if (PT == 2) __syncwarp();   // the even lane's copy serves its odd neighbour
-      unsigned long long base;
-      unsigned nvalid;
-      if (!chunk_range<CH>(ut, rpos, base, nvalid)) {   // block-uniform: end of work
-        more = false;
-        break;
-      }
-      if (rpos.r == 0) {   // the first warp to enter a unit prepares a later one
-        if (lane == 0 && sh::cas(claimed_a, (int)rpos.unit, (int)rpos.unit + 1) == (int)rpos.unit) {
+      if (rs.base >= rs.end) {     // (rare) the read stream enters a unit
+        stream_open(ut, rs);
+        if (rs.stop) {             // block-uniform: end of work
+          more = false;
+          break;
+        }
+        // the first warp to enter a unit prepares a later one
+        if (lane == 0 && sh::cas(claimed_a, (int)rs.unit, (int)rs.unit + 1) == (int)rs.unit) {
           tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
-          tk.unit = rpos.unit + ahead;
+          tk.unit = rs.unit + ahead;
           tk.pending = true;
         }
         __syncwarp();
+        ++rs.unit;
       }
-      rpos.advance(cps);
+      const unsigned long long base = rs.base;
+      const unsigned nvalid = rs.end - base >= (unsigned long long)CH ? (unsigned)CH : (unsigned)(rs.end - base);
+      rs.base += CH;
 
       // ---- step A1: this lane's PT scatterers, shared-memory stage -> registers; the slice is refilled at once ----
       Vec<PT> x, y, z, vx, vy, vz, s0;
@@ -387,7 +376,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
           s0.v[j] = v ? p.s0dA[i] : 0.0f;
         }
       }
-      if (++stg == (unsigned)S) stg = 0;
+      stg ^= 1u;
 
 #pragma unroll
       for (int gi = 0; gi < PT; gi += IL) {   // IL scatterers in flight per lane at a time

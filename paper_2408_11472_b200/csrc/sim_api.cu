@@ -223,7 +223,7 @@ cudaError_t plan_ws(sim_handle* h) {
   auto tiles_of = [&](int ww) { return smem(G, ww, 0); };
   while (w > 1 && tiles_of(w) + 2 * stage > budget) --w;
   int st = tiles_of(w) + 2 * stage <= budget ? (int)((budget - tiles_of(w)) / stage) : 2;
-  if (h->opt_window == 0 && st < 3) {
+  if (v3 && h->opt_window == 0 && st < 3) {
     // a third stage is worth more than the last bins of the window (measured on the 268M config; below 12 bins the
     // escapes take over)
     for (int w2 = w - 1; w2 >= 12 && w2 >= 3 * w / 4; --w2) {
@@ -234,7 +234,7 @@ cudaError_t plan_ws(sim_handle* h) {
       }
     }
   }
-  const int st_max = v3 ? 6 : 8;
+  const int st_max = v3 ? 6 : 2;   // variant 4: every lane copies one chunk ahead of its reads: two stages
   if (st > st_max) st = st_max;
   if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
   if (st < 2) st = 2;
