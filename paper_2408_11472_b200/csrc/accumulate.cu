@@ -89,11 +89,12 @@ __device__ __forceinline__ void publish_unit(const AccParams& p, const UnitTable
 }
 
 // A stream of chunks through the block's units (one for the copies, one for the reads): the current unit and the run
-// [base, end) of it that is left, in registers.  The unit table is consulted only when a unit is exhausted.
+// of it that is left, in registers.  The unit table is consulted only when a unit is exhausted.
 struct ChunkStream {
-  unsigned long long base, end;   // next chunk starts at base; base >= end: the unit is exhausted
-  unsigned unit;                  // index of the unit [base, end) belongs to (the next one to open when exhausted)
-  bool stop;                      // the end of work has been seen
+  unsigned long long base;   // the next chunk starts here
+  unsigned left;             // scatterers of the current unit not yet handed out (0: the unit is exhausted)
+  unsigned unit;             // index of the next unit to open
+  bool stop;                 // the end of work has been seen
 };
 
 // Opens unit s.unit (waits for its publication, all lanes together).  An empty unit is the end of work.
@@ -102,8 +103,10 @@ __device__ __forceinline__ void stream_open(const UnitTable& ut, ChunkStream& s)
   while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != s.unit + 1u) {
   }
   s.base = sh::ld64(ut.start0 + 8u * slot);
-  s.end = sh::ld64(ut.end0 + 8u * slot);
-  s.stop = s.end == 0ull;
+  const unsigned long long end = sh::ld64(ut.end0 + 8u * slot);
+  s.left = (unsigned)(end - s.base);   // a unit is shorter than 2^32 scatterers (sim_api.cu)
+  s.stop = end == 0ull;
+  ++s.unit;
 }
 
 // round(a * b) for |a b| <= 2^22 by the 1.5 * 2^23 trick (round to nearest even: unbiased), as an int
@@ -210,15 +213,12 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   PendingUnit tk{0u, 0u, false};
   // This lane's PT scatterers of the next chunk of the copy stream (7 x 16 bytes) -> its place in stage `st`; one commit
   // group per chunk, empty beyond the end of the input.  PT = 2 lanes pair up: the even lane copies for both.
-  ChunkStream cs{0ull, 0ull, 0u, false}, rs{0ull, 0ull, 0u, false};
+  ChunkStream cs{0ull, 0u, 0u, false}, rs{0ull, 0u, 0u, false};
   auto copy_chunk = [&](unsigned st) {
-    if (cs.base >= cs.end && !cs.stop) {   // (rare) the next unit
-      stream_open(ut, cs);
-      ++cs.unit;
-    }
+    if (cs.left == 0u && !cs.stop) stream_open(ut, cs);   // (rare) the next unit
     if (!cs.stop) {
-      const unsigned long long left = cs.end - cs.base;
-      const unsigned n4 = left >= (unsigned long long)CH ? (unsigned)CH : ((unsigned)left & ~3u);
+      const unsigned nv = min(cs.left, (unsigned)CH), n4 = nv & ~3u;
+      cs.left -= nv;
       const unsigned o4 = (slice_lo + e0) & ~3u;                    // first scatterer of this lane's 16-byte group
       if ((PT == 4 || !(lane & 1)) && o4 + 4u <= n4) {
         const unsigned dst = stage0 + st * kStageBytes + o4 * 4u;
@@ -331,23 +331,23 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       copy_chunk(stg ^ 1u);
       sh::cp_async_wait<1>();
       if (PT == 2) __syncwarp();   // the even lane's copy serves its odd neighbour
-      if (rs.base >= rs.end) {     // (rare) the read stream enters a unit
+      if (rs.left == 0u) {         // (rare) the read stream enters a unit
         stream_open(ut, rs);
         if (rs.stop) {             // block-uniform: end of work
           more = false;
           break;
         }
-        // the first warp to enter a unit prepares a later one
-        if (lane == 0 && sh::cas(claimed_a, (int)rs.unit, (int)rs.unit + 1) == (int)rs.unit) {
+        // the first warp to enter a unit (index rs.unit - 1) prepares a later one
+        if (lane == 0 && sh::cas(claimed_a, (int)rs.unit - 1, (int)rs.unit) == (int)rs.unit - 1) {
           tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
-          tk.unit = rs.unit + ahead;
+          tk.unit = rs.unit - 1u + ahead;
           tk.pending = true;
         }
         __syncwarp();
-        ++rs.unit;
       }
       const unsigned long long base = rs.base;
-      const unsigned nvalid = rs.end - base >= (unsigned long long)CH ? (unsigned)CH : (unsigned)(rs.end - base);
+      const unsigned nvalid = min(rs.left, (unsigned)CH);
+      rs.left -= nvalid;
       rs.base += CH;
 
       // ---- step A1: this lane's PT scatterers, shared-memory stage -> registers; the slice is refilled at once ----
@@ -607,8 +607,10 @@ __global__ void __launch_bounds__(256) acc_reference_kernel(AccParams p) {
 
 // T64 -> spectrum slot (complex64), T64 re-zeroed.  add != 0: the slot already holds earlier batches of this update
 // (SIM_ACC_APPEND).
-__global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add) {
+__global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add,
+                                                           unsigned int* __restrict__ counters) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) counters[kCtrTicket] = 0u;   // the scheduling counter of the next accumulation launch
   if (i >= cells) return;
   const double2 v = T64[i];
   float2 o = make_float2((float)v.x, (float)v.y);
@@ -621,8 +623,8 @@ __global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__
   if (v.x != 0.0 || v.y != 0.0) T64[i] = make_double2(0.0, 0.0);
 }
 
-cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches) {
-  acc_finalize_kernel<<<(cells + 255) / 256, 256, 0, st>>>(T64, T, cells, add ? 1 : 0);
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, unsigned int* counters, cudaStream_t st, int* launches) {
+  acc_finalize_kernel<<<(cells + 255) / 256, 256, 0, st>>>(T64, T, cells, add ? 1 : 0, counters);
   ++*launches;
   return cudaGetLastError();
 }
@@ -675,7 +677,8 @@ cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages,
 }
 
 // dbg: the same kernel writes (g0, k) per scatterer into p.dbg_g0 / p.dbg_k instead of accumulating.
-cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches) {
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, bool reset_ticket, cudaStream_t st,
+                              int* launches) {
   if (p.n == 0) return cudaSuccess;
   const int mode = acc_index_mode(p);
   AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, dbg);
@@ -684,8 +687,10 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
   // per launch: the limit is per function and per device, another handle may have set it for a smaller shape
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
-  if (e != cudaSuccess) return e;
+  if (reset_ticket) {   // (the finalize kernel leaves the scheduling counter at zero: only needed when none ran in between)
+    e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+  }
   const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
   const int grid = (int)(n_sc < (unsigned long long)blocks ? n_sc : (unsigned long long)blocks);
   k<<<grid, ncw * 32, smem, st>>>(p);

@@ -125,6 +125,7 @@ __device__ __forceinline__ float4 ldf4(unsigned a) {
 __device__ __forceinline__ void cp_async16(unsigned dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* src) { asm volatile("prefetch.global.L2 [%0];" ::"l"(src)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() {

@@ -91,6 +91,7 @@ struct sim_handle {
   size_t smem_per_sm;
   // stats
   uint64_t launches, scatterers_seen;
+  bool ticket_dirty;             // the scheduling counter may be non-zero (an accumulation launch without a finalize after it)
   std::string err;
 };
 
@@ -318,6 +319,7 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   }
   p.epoch_chunks = ec;
   const unsigned long long unit = (unsigned long long)ch * p.epoch_chunks;   // scheduling unit = whole epochs: a jump never splits one
+  if (sc > (1ull << 30)) sc = 1ull << 30;   // the kernels count the scatterers of a unit in 32 bits
   sc = (sc + unit - 1) / unit * unit;
   p.superchunk = sc;
   {  // scattered visiting order: dark and illuminated parts of the scene are in flight at the same time, so the
@@ -352,8 +354,9 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
   int l = 0;
   cudaError_t e = h->opt_variant == 3   ? launch_accumulate_ws3(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, h->stream, &l)
                   : h->opt_variant == 0 ? launch_reference(p, h->sm_count, h->stream, &l)
-                                        : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->stream, &l);
+                                        : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->ticket_dirty, h->stream, &l);
   h->launches += l;
+  if (l) h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
 }
@@ -363,9 +366,10 @@ int do_finalize(sim_handle* h, float2* T, bool add) {
   if (h->opt_variant == 3) return SIM_OK;
   int l = 0;
   cudaError_t e = launch_finalize(reinterpret_cast<double2*>(h->ws + h->lay.t64_off), T, h->cfg.n_gates * h->cfg.n_doppler, add,
-                                  h->stream, &l);
+                                  counters(h), h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "finalize launch");
+  h->ticket_dirty = false;
   return SIM_OK;
 }
 
@@ -486,6 +490,7 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->ws_blocks_per_sm = 0;
   h->launches = 0;
   h->scatterers_seen = 0;
+  h->ticket_dirty = true;
   int v = 0;
   e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cfg->device);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)"); }
@@ -738,8 +743,9 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   int l = 0;
   // the production kernel itself, exporting its indices instead of accumulating (variant 3: its own index kernel)
   cudaError_t e = h->opt_variant == 3 ? launch_indices3(p, d_gate0, d_bin, h->sm_count, h->stream, &l)
-                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, h->stream, &l);
+                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, true, h->stream, &l);
   h->launches += l;
+  h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
   return SIM_OK;
 }

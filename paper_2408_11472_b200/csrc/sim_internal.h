@@ -86,9 +86,10 @@ int acc_chunk(int ncw, int pt);
 size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages);
 bool acc_supported(int ncw, int pt, int il);
 cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
-cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches);
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, bool reset_ticket, cudaStream_t st,
+                              int* launches);
 cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches);
-cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches);
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, unsigned int* counters, cudaStream_t st, int* launches);
 // round-1 production kernel, kept for A/B (accumulate_ws3.cu): producer warp + drain warp + ncw compute warps
 size_t acc_ws3_smem_bytes(int G, int W, int ncw, int pt, int stages);
 bool acc_ws3_supported(int ncw, int pt, int il);
