@@ -100,8 +100,7 @@ struct ChunkStream {
 // Opens unit s.unit (waits for its publication, all lanes together).  An empty unit is the end of work.
 __device__ __forceinline__ void stream_open(const UnitTable& ut, ChunkStream& s) {
   const unsigned slot = s.unit & (kRing - 1);
-  while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != s.unit + 1u) {
-  }
+  while ((unsigned)sh::ld_acquire(ut.seq0 + 4u * slot) != s.unit + 1u) __nanosleep(64);
   s.base = sh::ld64(ut.start0 + 8u * slot);
   const unsigned long long end = sh::ld64(ut.end0 + 8u * slot);
   s.left = (unsigned)(end - s.base);   // a unit is shorter than 2^32 scatterers (sim_api.cu)
@@ -213,12 +212,31 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   PendingUnit tk{0u, 0u, false};
   // This lane's PT scatterers of the next chunk of the copy stream (7 x 16 bytes) -> its place in stage `st`; one commit
   // group per chunk, empty beyond the end of the input.  PT = 2 lanes pair up: the even lane copies for both.
-  ChunkStream cs{0ull, 0u, 0u, false}, rs{0ull, 0u, 0u, false};
+  // One stream of chunks: the chunk copied in an iteration is the one read in the next (two stages).
+  ChunkStream cs{0ull, 0u, 0u, false};
+  unsigned long long rd_base = 0ull;   // the chunk to read next (copied one iteration ago): first scatterer,
+  unsigned rd_nv = 0u;                 // valid count (0: none, the end of work has been reached)
+  unsigned long long cp_base = 0ull;   // the chunk copied last
+  unsigned cp_nv = 0u;
   auto copy_chunk = [&](unsigned st) {
-    if (cs.left == 0u && !cs.stop) stream_open(ut, cs);   // (rare) the next unit
+    cp_nv = 0u;
+    if (cs.left == 0u && !cs.stop) {   // (rare) the next unit
+      stream_open(ut, cs);
+      // the first warp to enter a unit (index cs.unit - 1) prepares a later one
+      if (!cs.stop) {
+        if (lane == 0 && sh::cas(claimed_a, (int)cs.unit - 1, (int)cs.unit) == (int)cs.unit - 1) {
+          tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
+          tk.unit = cs.unit - 1u + ahead;
+          tk.pending = true;
+        }
+        __syncwarp();
+      }
+    }
     if (!cs.stop) {
       const unsigned nv = min(cs.left, (unsigned)CH), n4 = nv & ~3u;
       cs.left -= nv;
+      cp_base = cs.base;
+      cp_nv = nv;
       const unsigned o4 = (slice_lo + e0) & ~3u;                    // first scatterer of this lane's 16-byte group
       if ((PT == 4 || !(lane & 1)) && o4 + 4u <= n4) {
         const unsigned dst = stage0 + st * kStageBytes + o4 * 4u;
@@ -236,6 +254,8 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     sh::cp_async_commit();
   };
   copy_chunk(0u);   // chunk 0 is in flight (two stages: the copies run one chunk ahead of the reads)
+  rd_base = cp_base;
+  rd_nv = cp_nv;
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
@@ -293,6 +313,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       const unsigned b = dpend & 1u;
       if (sh::ld_acquire(complete0 + 4u * b) <= (int)(dpend >> 1)) {
         if (!block) return;
+        __nanosleep(256);   // a warp that is ahead must not take issue slots from the ones it waits for
         continue;
       }
       drain_share(dpend);
@@ -315,8 +336,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     const unsigned slot = slot0 + 4u * kSlotInts * (e & 3u);
     if (!DBG && e >= 2) {   // the tile of epoch e-2 must be back: this warp's own share first, then everybody else's
       try_drain(e - 1u, true);
-      while (sh::ld_acquire(drained0 + 4u * (e & 1u)) < (int)(e >> 1)) {
-      }
+      while (sh::ld_acquire(drained0 + 4u * (e & 1u)) < (int)(e >> 1)) __nanosleep(256);
     }
     // tile base of this lane's first reduction, the +1 row offset of the padded tile folded in
     const unsigned tile_b = tile0 + (e & 1u) * tile_bytes + (unsigned)RS4 + off_b0;
@@ -331,24 +351,14 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       copy_chunk(stg ^ 1u);
       sh::cp_async_wait<1>();
       if (PT == 2) __syncwarp();   // the even lane's copy serves its odd neighbour
-      if (rs.left == 0u) {         // (rare) the read stream enters a unit
-        stream_open(ut, rs);
-        if (rs.stop) {             // block-uniform: end of work
-          more = false;
-          break;
-        }
-        // the first warp to enter a unit (index rs.unit - 1) prepares a later one
-        if (lane == 0 && sh::cas(claimed_a, (int)rs.unit - 1, (int)rs.unit) == (int)rs.unit - 1) {
-          tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
-          tk.unit = rs.unit - 1u + ahead;
-          tk.pending = true;
-        }
-        __syncwarp();
+      if (rd_nv == 0u) {           // block-uniform: end of work
+        more = false;
+        break;
       }
-      const unsigned long long base = rs.base;
-      const unsigned nvalid = min(rs.left, (unsigned)CH);
-      rs.left -= nvalid;
-      rs.base += CH;
+      const unsigned long long base = rd_base;
+      const unsigned nvalid = rd_nv;
+      rd_base = cp_base;
+      rd_nv = cp_nv;
 
       // ---- step A1: this lane's PT scatterers, shared-memory stage -> registers; the slice is refilled at once ----
       Vec<PT> x, y, z, vx, vy, vz, s0;
@@ -508,8 +518,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
             }
             __syncwarp();
           } else if (st == kSlotClaimed) {
-            while (sh::ld_acquire(slot + 4 * kSlotState) != kSlotReady) {
-            }
+            while (sh::ld_acquire(slot + 4 * kSlotState) != kSlotReady) __nanosleep(64);
           }
           k0 = sh::ld(slot + 4 * kSlotK0);
           const int ex = sh::ld(slot + 4 * kSlotEx);
