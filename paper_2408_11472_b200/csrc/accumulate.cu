@@ -51,9 +51,23 @@ enum { kSlotUnset = 0, kSlotClaimed = 1, kSlotReady = 2 };
 // scheduling-unit table in shared memory (ring): first scatterer, end, sequence number (= unit index + 1 once published)
 int acc_chunk(int ncw, int pt) { return ncw * 32 * pt; }
 
-static int acc_row_stride(int W) { return (W + 3) & ~3; }   // words per tile row: 16-byte rows for the drain's vector loads
+// Tile layout (bank behaviour simulated on the nadir and PM scenes and confirmed by ncu, profiles/): words per row = 4
+// mod 8 (rows g .. g + 7 of one bin then sit in eight different banks), words per plane = 2 mod 32 (the four planes
+// that the lanes of one reduction instruction are spread over do not alias bank for bank): 4.1 wavefronts per
+// reduction instruction on the white-noise scene against 7.2 for rows of 12 and planes of 12 mod 32, and 9.4 without
+// the lane rotation.
+int acc_row_stride(int W) {
+  int rs = (W + 1) & ~1;
+  while ((rs & 7) != 4) rs += 2;
+  return rs;
+}
+int acc_plane_words(int G, int W) {
+  int w = (G + 1) * acc_row_stride(W);
+  while ((w & 31) != 2) w += 2;
+  return w;
+}
 
-size_t acc_tile_bytes(int G, int W) { return (size_t)4 * (G + 1) * acc_row_stride(W) * sizeof(int); }   // one tile: four planes
+size_t acc_tile_bytes(int G, int W) { return (size_t)4 * acc_plane_words(G, W) * sizeof(int); }   // one tile: four planes
 
 size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages) {
   return (size_t)stages * 7 * acc_chunk(ncw, pt) * sizeof(float) + 2 * acc_tile_bytes(G, W);
@@ -171,10 +185,10 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int S = p.stages, EC = p.epoch_chunks;
-  const int G = p.G, W = p.W, RS = (W + 3) & ~3;
+  const int G = p.G, W = p.W, RS = p.row_words;
   const unsigned stage0 = sh::addr(smem_raw);
   const unsigned tile0 = stage0 + (unsigned)S * kStageBytes;     // int [2 tiles][4 planes: L.re, L.im, U.re, U.im][G + 1][RS]
-  const unsigned plane_bytes = (unsigned)((G + 1) * RS) * 4u, tile_bytes = 4u * plane_bytes;
+  const unsigned plane_bytes = (unsigned)p.plane_words * 4u, tile_bytes = 4u * plane_bytes;
   const UnitTable ut{sh::addr(&s_ustart[0]), sh::addr(&s_uend[0]), sh::addr(&s_useq[0])};
   const unsigned claimed_a = sh::addr(&s_claimed);
   const unsigned tcount0 = sh::addr(&s_tcount[0]), drained0 = sh::addr(&s_drained[0]);
@@ -260,9 +274,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
   // halves of row g (g0 = g - 1); row 0 of L and row G of U only collect the halves that fall outside the window: never
-  // read, never zeroed.  One lane = four consecutive bins of one gate: four 16-byte loads.
+  // read, never zeroed.  One lane = two consecutive bins of one gate: four 8-byte loads.
   const int g_lo = (int)(((long long)G * warp) / NCW), g_hi = (int)(((long long)G * (warp + 1)) / NCW);
-  const int quads = RS >> 2;
+  const int pairs = RS >> 1;
   auto drain_share = [&](unsigned d) {
     const unsigned b = d & 1u;
     const unsigned slot = slot0 + 4u * kSlotInts * (d & 3u);
@@ -270,24 +284,23 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       const int k0 = pmod(sh::ld(slot + 4 * kSlotK0), p.N), ex = sh::ld(slot + 4 * kSlotEx);
       const double inv_s = __hiloint2double((1023 - ex) << 20, 0);
       const unsigned tile = tile0 + b * tile_bytes;
-      const int nitem = (g_hi - g_lo) * quads;
+      const int nitem = (g_hi - g_lo) * pairs;
       for (int it = lane; it < nitem; it += 32) {
-        const int g = g_lo + it / quads, q4 = (it % quads) * 4;
-        const unsigned aL = tile + 4u * (unsigned)((g + 1) * RS + q4), aU = tile + 2u * plane_bytes + 4u * (unsigned)(g * RS + q4);
-        const int4 lr = sh::ld4(aL), li = sh::ld4(aL + plane_bytes), ur = sh::ld4(aU), ui = sh::ld4(aU + plane_bytes);
-        const int any = lr.x | lr.y | lr.z | lr.w | li.x | li.y | li.z | li.w | ur.x | ur.y | ur.z | ur.w | ui.x | ui.y | ui.z | ui.w;
-        if (any) {
-          const int4 z4 = make_int4(0, 0, 0, 0);
-          sh::st4(aL, z4);
-          sh::st4(aL + plane_bytes, z4);
-          sh::st4(aU, z4);
-          sh::st4(aU + plane_bytes, z4);
-          const int re[4] = {lr.x + ur.x, lr.y + ur.y, lr.z + ur.z, lr.w + ur.w};
-          const int im[4] = {li.x + ui.x, li.y + ui.y, li.z + ui.z, li.w + ui.w};
+        const int g = g_lo + it / pairs, q2 = (it % pairs) * 2;
+        const unsigned aL = tile + 4u * (unsigned)((g + 1) * RS + q2), aU = tile + 2u * plane_bytes + 4u * (unsigned)(g * RS + q2);
+        const int2 lr = sh::ld2(aL), li = sh::ld2(aL + plane_bytes), ur = sh::ld2(aU), ui = sh::ld2(aU + plane_bytes);
+        if (lr.x | lr.y | li.x | li.y | ur.x | ur.y | ui.x | ui.y) {
+          const int2 z2 = make_int2(0, 0);
+          sh::st2(aL, z2);
+          sh::st2(aL + plane_bytes, z2);
+          sh::st2(aU, z2);
+          sh::st2(aU + plane_bytes, z2);
+          const int re[2] = {lr.x + ur.x, lr.y + ur.y};
+          const int im[2] = {li.x + ui.x, li.y + ui.y};
   #pragma unroll
-          for (int c = 0; c < 4; ++c) {
+          for (int c = 0; c < 2; ++c) {
             if (re[c] | im[c]) {   // (columns >= W are never written)
-              int bin = k0 + q4 + c;
+              int bin = k0 + q2 + c;
               bin -= bin >= p.N ? p.N : 0;
               double* t = reinterpret_cast<double*>(p.T64 + (size_t)g * p.N + bin);
               atomicAdd(t, (double)re[c] * inv_s);
@@ -523,7 +536,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
           k0 = sh::ld(slot + 4 * kSlotK0);
           const int ex = sh::ld(slot + 4 * kSlotEx);
           s = __int_as_float((ex + 127) << 23);
-          sS = sw_lu ? -s : s;
+          sS = (sw_lu ? -s : s) * p.w_scale;
           sO = sw_lu ? s : 0.0f;
           lo_bits = (11 - ex + 127) << 23;                    // bits of 2^11 / s
           have = true;
@@ -536,8 +549,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
         for (int j = 0; j < IL; ++j) {
           const int kw = k[j] - k0;
           const bool fits = ok[j] && !near[j] && (unsigned)kw < (unsigned)W && (unsigned)(ab[j] - lo_bits) <= fx_span;
-          const float w1 = (float)(fx[j].gfx & (kFxOne - 1)) * p.w_scale;
-          const float wAs = fmaf(w1, sS, sO), wBs = s - wAs;             // (w1, w0) s, or (w0, w1) s on swapped lanes
+          const float wAs = fmaf((float)(fx[j].gfx & (kFxOne - 1)), sS, sO), wBs = s - wAs;             // (w1, w0) s, or (w0, w1) s on swapped lanes
           const float a0 = sw_ri ? c[j].y : c[j].x, a1 = sw_ri ? c[j].x : c[j].y;
           const unsigned adr = tile_b + (unsigned)(g0[j] * RS4 + 4 * kw);
           if (fits) {
@@ -662,7 +674,7 @@ static AccKernel acc_kernel_ptr(int ncw, int pt, int il, int mode, bool dbg) {
          : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, false>            \
                                      : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, false>;               \
   }
-  ACC_CASE(8, 4, 4) ACC_CASE(8, 2, 2) ACC_CASE(16, 4, 4)
+  ACC_CASE(8, 4, 4) ACC_CASE(8, 4, 2) ACC_CASE(8, 2, 2) ACC_CASE(16, 4, 4)
 #undef ACC_CASE
   return nullptr;
 }

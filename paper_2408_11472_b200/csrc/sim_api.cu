@@ -219,7 +219,7 @@ cudaError_t plan_ws(sim_handle* h) {
   budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
   if (budget > h->smem_optin - 1024) budget = h->smem_optin - 1024;
   const size_t stage = smem(0, 0, 1) - smem(0, 0, 0);
-  int w = h->opt_window > 0 ? h->opt_window : 16;
+  int w = h->opt_window > 0 ? h->opt_window : (v3 ? 16 : 20);
   if (w > N) w = N;
   auto tiles_of = [&](int ww) { return smem(G, ww, 0); };
   while (w > 1 && tiles_of(w) + 2 * stage > budget) --w;
@@ -239,6 +239,7 @@ cudaError_t plan_ws(sim_handle* h) {
   if (st > st_max) st = st_max;
   if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
   if (st < 2) st = 2;
+  if (!v3 && h->opt_window == 0 && acc_row_stride(w) <= N) w = acc_row_stride(w);   // the padding columns of a row are free
   h->ws_W = w;
   h->ws_stages = st;
   int b = 1;
@@ -308,6 +309,8 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
     if (fair < (unsigned long long)ec) ec = fair > 0 ? (int)fair : 1;
   }
   p.W = h->ws_W;
+  p.row_words = acc_row_stride(p.W);
+  p.plane_words = acc_plane_words(h->cfg.n_gates, p.W);
   p.stages = h->ws_stages;
   p.wait_hint = (unsigned)h->opt_wait_hint;
   {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31

@@ -60,6 +60,7 @@ struct AccParams {
   unsigned int* counters; // kNumCounters device words
   unsigned long long superchunk; // scatterers per scheduling unit (whole fixed-point epochs)
   int W;                  // Doppler bins of the shared-memory window
+  int row_words, plane_words;   // production kernel: tile layout (accumulate.cu)
   int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
   int fx_cap, fx_target;     // block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
   unsigned long long sc_stride;  // scheduling unit visited by ticket t is (t * sc_stride) mod n_units (coprime)
@@ -83,6 +84,8 @@ struct SynParams {
 
 // production kernel (accumulate.cu): ncw compute warps + 1 drain warp per block, pt scatterers per lane per chunk
 int acc_chunk(int ncw, int pt);
+int acc_row_stride(int W);
+int acc_plane_words(int G, int W);
 size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages);
 bool acc_supported(int ncw, int pt, int il);
 cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
