@@ -217,7 +217,7 @@ cudaError_t plan_ws(sim_handle* h) {
   const int target = ncw <= 8 ? 2 : 1;                              // blocks per SM the register budget allows
   size_t budget = h->smem_per_sm / target;
   budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
-  if (budget > h->smem_optin - 1024) budget = h->smem_optin - 1024;
+  if (budget > h->smem_optin - 4096) budget = h->smem_optin - 4096;   // the kernels' static shared memory (< 3 KB) counts against the opt-in limit
   const size_t stage = smem(0, 0, 1) - smem(0, 0, 0);
   int w = h->opt_window > 0 ? h->opt_window : (v3 ? 16 : 20);
   if (w > N) w = N;
