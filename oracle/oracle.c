@@ -21,6 +21,11 @@
  *                            "Summing the weighted time-long signals in the corresponding cells of Y"
  *                            (PAPER.md:100-101); eq. (1) at PAPER.md:61, W_i(x) = (1 - |i-x|/n_fast)^(1/2).
  *
+ *   O1' oracle_spectrum_lut -- O1 with the antenna gain read from a complex table on a u-v grid by bilinear
+ *                            interpolation ("all antenna patterns ... are computed and recorded on a
+ *                            u-v grid.  The complex values ... at each facet are then obtained through interpolation
+ *                            in the u-v grid"; reading R9 fixes the frame, the interpolation and the edge rule).
+ *
  *   R   oracle_regular    -- the REGULAR mode: per-pulse complex sum of all scatterers per
  *                            range gate, surface "updated at each PRF" (reading R5).
  *
@@ -28,6 +33,9 @@
  * special case, Parseval, brute-force regular-mode sum, an independent numpy restatement); the
  * pulse-pair Doppler mode by tests/test_oracle_pulse_pair.py (the literal arg(C_{i+1} C_i^*) estimator at
  * 50 digits, the analytic f_D plus its closed-form second-order term, aliasing).
+ * The table gain by tests/test_oracle_lut.py (constant table = isotropic, a table linear in u and v
+ * reproduced exactly, a finely sampled Gaussian against the analytic gain within the interpolation bound,
+ * mpmath closed form of single scatterers, the frame and the edge rule).
  * Parity unpinned BY THE PAPER (fixed only by DESIGN.md readings): the analytic antenna gain
  * G(theta) (A10), the tail rule for a missing successor spectrum (A3), the nearest-bin rule (A7).
  *
@@ -149,13 +157,55 @@ static void unit_boresight(const oracle_sat *s, double b[3]) {
   b[2] = s->boresight[2] / n;
 }
 
-/* O1 for scatterers [lo,hi) into T (complex128 as [G][N][2], bin fastest). */
-static void spectrum_range(const oracle_config *c, const oracle_sat *s, int64_t lo, int64_t hi,
+/* Antenna pattern recorded on a u-v grid (reading R9).
+ *   Frame: b = unit boresight; e1 = unit vector of vel - (vel.b) b (along track, normal to the boresight);
+ *   e2 = b x e1.  Direction cosines of the line of sight d = r_p - r_sat:  u = d.e1 / R,  v = d.e2 / R.
+ *   Table: complex64 values G[j][i] (interleaved re, im; i fastest) at u_i = u0 + i du, v_j = v0 + j dv.
+ *   Gain at (u, v): bilinear interpolation between the four surrounding nodes; (u, v) outside
+ *   [u0, u0 + (nu-1) du] x [v0, v0 + (nv-1) dv] (or NaN) is outside the recorded pattern: gain 0. */
+typedef struct {
+  const float *table; /* [nv][nu][2] */
+  int32_t nu, nv;
+  double u0, du, v0, dv;
+} oracle_lut;
+
+/* returns 0 when (u, v) is outside the table */
+static int lut_gain(const oracle_lut *L, double u, double v, double *gre, double *gim) {
+  const double fu = (u - L->u0) / L->du, fv = (v - L->v0) / L->dv;
+  if (!(fu >= 0.0 && fu <= (double)(L->nu - 1) && fv >= 0.0 && fv <= (double)(L->nv - 1))) return 0;
+  int i = (int)floor(fu), j = (int)floor(fv);
+  if (i > L->nu - 2) i = L->nu - 2; /* the last node belongs to the last cell */
+  if (j > L->nv - 2) j = L->nv - 2;
+  const double a = fu - (double)i, bb = fv - (double)j;
+  const float *t00 = L->table + 2 * ((int64_t)j * L->nu + i);
+  const float *t01 = t00 + 2, *t10 = t00 + 2 * (int64_t)L->nu, *t11 = t10 + 2;
+  const double w00 = (1.0 - a) * (1.0 - bb), w01 = a * (1.0 - bb), w10 = (1.0 - a) * bb, w11 = a * bb;
+  *gre = w00 * (double)t00[0] + w01 * (double)t01[0] + w10 * (double)t10[0] + w11 * (double)t11[0];
+  *gim = w00 * (double)t00[1] + w01 * (double)t01[1] + w10 * (double)t10[1] + w11 * (double)t11[1];
+  return 1;
+}
+
+/* antenna frame of reading R9; returns 0 when the velocity is parallel to the boresight (no along-track axis) */
+static int antenna_frame(const oracle_sat *s, const double b[3], double e1[3], double e2[3]) {
+  const double vb = s->vel[0] * b[0] + s->vel[1] * b[1] + s->vel[2] * b[2];
+  double t[3] = {s->vel[0] - vb * b[0], s->vel[1] - vb * b[1], s->vel[2] - vb * b[2]};
+  const double n = sqrt(t[0] * t[0] + t[1] * t[1] + t[2] * t[2]);
+  if (!(n > 0.0)) return 0;
+  for (int i = 0; i < 3; ++i) e1[i] = t[i] / n;
+  e2[0] = b[1] * e1[2] - b[2] * e1[1];
+  e2[1] = b[2] * e1[0] - b[0] * e1[2];
+  e2[2] = b[0] * e1[1] - b[1] * e1[0];
+  return 1;
+}
+
+/* O1 for scatterers [lo,hi) into T (complex128 as [G][N][2], bin fastest).  lut == NULL: analytic gain. */
+static void spectrum_range(const oracle_config *c, const oracle_sat *s, const oracle_lut *lut, int64_t lo, int64_t hi,
                            const float *x, const float *y, const float *z, const float *vx,
                            const float *vy, const float *vz, const float *s0dA, double *T) {
-  double inv_dR, two_over_lambda, cD, b[3];
+  double inv_dR, two_over_lambda, cD, b[3], e1[3] = {0, 0, 0}, e2[3] = {0, 0, 0};
   constants(c, &inv_dR, &two_over_lambda, &cD);
   unit_boresight(s, b);
+  if (lut && !antenna_frame(s, b, e1, e2)) return;
   const int G = c->n_gates, N = c->n_doppler;
   for (int64_t p = lo; p < hi; ++p) {
     if (!(s0dA[p] > 0.0f)) continue; /* s0dA <= 0 (or NaN) contributes nothing */
@@ -167,11 +217,17 @@ static void spectrum_range(const oracle_config *c, const oracle_sat *s, int64_t 
     const double cy = g.dz * b[0] - g.dx * b[2];
     const double cz = g.dx * b[1] - g.dy * b[0];
     const double sin2 = (cx * cx + cy * cy + cz * cz) / g.R2;
-    const double gain = exp(-c->antenna_alpha * sin2);
-    /* C_i: sqrt(sigma0 dA) G(theta) / R^2 exp(-i 4 pi R / lambda)  (north_star) */
-    const double A = sqrt((double)s0dA[p]) * gain / g.R2;
-    const double re = A * cos(TWO_PI * g.fr);
-    const double im = -A * sin(TWO_PI * g.fr);
+    double gre = exp(-c->antenna_alpha * sin2), gim = 0.0;
+    if (lut) { /* complex pattern value interpolated in the u-v grid */
+      const double u = (g.dx * e1[0] + g.dy * e1[1] + g.dz * e1[2]) / g.R;
+      const double v = (g.dx * e2[0] + g.dy * e2[1] + g.dz * e2[2]) / g.R;
+      if (!lut_gain(lut, u, v, &gre, &gim)) continue;
+    }
+    /* C_i: sqrt(sigma0 dA) G / R^2 exp(-i 4 pi R / lambda)  (north_star) */
+    const double A = sqrt((double)s0dA[p]) / g.R2;
+    const double pr = cos(TWO_PI * g.fr), pi_ = -sin(TWO_PI * g.fr);
+    const double re = A * (gre * pr - gim * pi_);
+    const double im = A * (gre * pi_ + gim * pr);
     /* rasterize: two-gate linear split (A8), halves outside the window dropped */
     if (g.g0 >= 0 && g.g0 < G) {
       double *t = T + 2 * ((int64_t)g.g0 * N + g.k);
@@ -189,14 +245,14 @@ static void spectrum_range(const oracle_config *c, const oracle_sat *s, int64_t 
 /* O1. T is [G][N] complex128 (interleaved re,im).  accumulate != 0 adds to T (the paper's tiles,
  * PAPER.md:39); otherwise T is zeroed first.  nthreads <= 1: one plain loop.  nthreads > 1:
  * contiguous scatterer ranges per thread into private grids, summed in thread order. */
-int oracle_spectrum(const oracle_config *c, const oracle_sat *s, int64_t n, const float *x,
-                    const float *y, const float *z, const float *vx, const float *vy,
-                    const float *vz, const float *s0dA, double *T, int accumulate, int nthreads) {
+static int spectrum_any(const oracle_config *c, const oracle_sat *s, const oracle_lut *lut, int64_t n, const float *x,
+                        const float *y, const float *z, const float *vx, const float *vy,
+                        const float *vz, const float *s0dA, double *T, int accumulate, int nthreads) {
   if (!c || !s || !T || n < 0 || c->n_gates < 1 || c->n_doppler < 1) return -1;
   const int64_t cells = (int64_t)c->n_gates * c->n_doppler;
   if (!accumulate) memset(T, 0, (size_t)cells * 2 * sizeof(double));
   if (nthreads <= 1) {
-    spectrum_range(c, s, 0, n, x, y, z, vx, vy, vz, s0dA, T);
+    spectrum_range(c, s, lut, 0, n, x, y, z, vx, vy, vz, s0dA, T);
     return 1;
   }
 #ifdef _OPENMP
@@ -207,16 +263,35 @@ int oracle_spectrum(const oracle_config *c, const oracle_sat *s, int64_t n, cons
     const int t = omp_get_thread_num();
     const int nt = omp_get_num_threads();
     const int64_t lo = n * t / nt, hi = n * (t + 1) / nt;
-    spectrum_range(c, s, lo, hi, x, y, z, vx, vy, vz, s0dA, priv + (size_t)t * cells * 2);
+    spectrum_range(c, s, lut, lo, hi, x, y, z, vx, vy, vz, s0dA, priv + (size_t)t * cells * 2);
   }
   for (int t = 0; t < nthreads; ++t)
     for (int64_t j = 0; j < cells * 2; ++j) T[j] += priv[(size_t)t * cells * 2 + j];
   free(priv);
   return nthreads;
 #else
-  spectrum_range(c, s, 0, n, x, y, z, vx, vy, vz, s0dA, T);
+  spectrum_range(c, s, lut, 0, n, x, y, z, vx, vy, vz, s0dA, T);
   return 1;
 #endif
+}
+
+int oracle_spectrum(const oracle_config *c, const oracle_sat *s, int64_t n, const float *x,
+                    const float *y, const float *z, const float *vx, const float *vy,
+                    const float *vz, const float *s0dA, double *T, int accumulate, int nthreads) {
+  return spectrum_any(c, s, NULL, n, x, y, z, vx, vy, vz, s0dA, T, accumulate, nthreads);
+}
+
+/* O1 with the tabulated antenna pattern (reading R9).  -3: bad table or no antenna frame. */
+int oracle_spectrum_lut(const oracle_config *c, const oracle_sat *s, const oracle_lut *lut, int64_t n, const float *x,
+                        const float *y, const float *z, const float *vx, const float *vy,
+                        const float *vz, const float *s0dA, double *T, int accumulate, int nthreads) {
+  if (!lut || !lut->table || lut->nu < 2 || lut->nv < 2 || !(lut->du > 0.0) || !(lut->dv > 0.0)) return -3;
+  if (s) {
+    double b[3], e1[3], e2[3];
+    unit_boresight(s, b);
+    if (!antenna_frame(s, b, e1, e2)) return -3;
+  }
+  return spectrum_any(c, s, lut, n, x, y, z, vx, vy, vz, s0dA, T, accumulate, nthreads);
 }
 
 /* Indices only (canonical sequence).  g0[p] in [-1, G-1], k[p] in [0, N); a dropped scatterer

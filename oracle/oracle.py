@@ -46,6 +46,18 @@ class OracleSat(C.Structure):
     ]
 
 
+class OracleLut(C.Structure):
+    _fields_ = [
+        ("table", C.POINTER(C.c_float)),
+        ("nu", C.c_int32),
+        ("nv", C.c_int32),
+        ("u0", C.c_double),
+        ("du", C.c_double),
+        ("v0", C.c_double),
+        ("dv", C.c_double),
+    ]
+
+
 def build(force: bool = False) -> str:
     """Compile oracle.c -> liboracle.so (gcc, -ffp-contract=off, OpenMP)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
@@ -69,6 +81,9 @@ def lib():
         L.oracle_spectrum.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
                                       fp, fp, fp, fp, fp, fp, fp, dp, C.c_int, C.c_int]
         L.oracle_spectrum.restype = C.c_int
+        L.oracle_spectrum_lut.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.POINTER(OracleLut), C.c_int64,
+                                          fp, fp, fp, fp, fp, fp, fp, dp, C.c_int, C.c_int]
+        L.oracle_spectrum_lut.restype = C.c_int
         L.oracle_indices.argtypes = [C.POINTER(OracleConfig), C.POINTER(OracleSat), C.c_int64,
                                      fp, fp, fp, fp, fp, fp, ip, ip]
         L.oracle_indices.restype = C.c_int
@@ -133,6 +148,22 @@ def spectrum(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz, s0dA, out=N
     if rc < 0:
         raise RuntimeError(f"oracle_spectrum failed: {rc}")
     return out, rc
+
+
+def spectrum_lut(cfg: OracleConfig, sat: OracleSat, table, u0, du, v0, dv, x, y, z, vx, vy, vz, s0dA, nthreads=1):
+    """O1 with the antenna gain interpolated in a complex u-v table [nv][nu] (reading R9)."""
+    tab = np.ascontiguousarray(table, dtype=np.complex64)
+    assert tab.ndim == 2
+    lut = OracleLut(tab.view(np.float32).ctypes.data_as(C.POINTER(C.c_float)), tab.shape[1], tab.shape[0],
+                    float(u0), float(du), float(v0), float(dv))
+    arrs = [_f32(a) for a in (x, y, z, vx, vy, vz, s0dA)]
+    n = arrs[0][0].size
+    out = np.zeros((cfg.n_gates, cfg.n_doppler), dtype=np.complex128)
+    rc = lib().oracle_spectrum_lut(C.byref(cfg), C.byref(sat), C.byref(lut), n, *[a[1] for a in arrs],
+                                   out.ctypes.data_as(C.POINTER(C.c_double)), 0, int(nthreads))
+    if rc < 0:
+        raise RuntimeError(f"oracle_spectrum_lut failed: {rc}")
+    return out
 
 
 def indices(cfg: OracleConfig, sat: OracleSat, x, y, z, vx, vy, vz):

@@ -36,9 +36,21 @@ def closed_form(scat, sat_pos, sat_vel, boresight, range_gate0, lam, prf, dR, N,
     return {"R": R, "gf": gf, "fD": fD, "kf": kf, "fr": fr, "gain": gain, "A": A, "c": complex(c)}
 
 
+def uv_frame(sat_vel, boresight):
+    """Antenna frame of DESIGN.md reading R9, restated: b unit boresight, e1 the unit along-track
+    vector normal to b, e2 = b x e1."""
+    b = np.asarray(boresight, np.float64)
+    b = b / np.linalg.norm(b)
+    v = np.asarray(sat_vel, np.float64)
+    t = v - np.dot(v, b) * b
+    e1 = t / np.linalg.norm(t)
+    return b, e1, np.cross(b, e1)
+
+
 def numpy_spectrum(x, y, z, vx, vy, vz, s0dA, sat_pos, sat_vel, boresight, range_gate0, lam, prf,
-                   dR, G, N, alpha):
-    """[G][N] complex128 spectrum, vectorised; phases reduced in 80-bit long double."""
+                   dR, G, N, alpha, gain_fn=None):
+    """[G][N] complex128 spectrum, vectorised; phases reduced in 80-bit long double.
+    gain_fn(u, v) -> complex gain replaces the analytic pattern (u, v: direction cosines in uv_frame)."""
     L = np.longdouble
     d = np.stack([np.asarray(x, L) - L(sat_pos[0]), np.asarray(y, L) - L(sat_pos[1]),
                   np.asarray(z, L) - L(sat_pos[2])])
@@ -59,7 +71,13 @@ def numpy_spectrum(x, y, z, vx, vy, vz, s0dA, sat_pos, sat_vel, boresight, range
     b = b / np.linalg.norm(b)
     cr = np.cross(d.astype(np.float64).T, b)
     sin2 = (cr * cr).sum(1) / (R * R).astype(np.float64)
-    A = np.sqrt(np.asarray(s0dA, np.float64)) * np.exp(-alpha * sin2) / (R * R).astype(np.float64)
+    if gain_fn is None:
+        gain = np.exp(-alpha * sin2)
+    else:
+        _, e1, e2 = uv_frame(sat_vel, boresight)
+        d64 = d.astype(np.float64).T
+        gain = gain_fn(d64 @ e1 / R.astype(np.float64), d64 @ e2 / R.astype(np.float64))
+    A = np.sqrt(np.asarray(s0dA, np.float64)) * gain / (R * R).astype(np.float64)
     A = np.where(np.asarray(s0dA) > 0, A, 0.0)
     c = A * np.exp(-2j * np.pi * fr)
     T = np.zeros((G, N), np.complex128)
