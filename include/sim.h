@@ -177,6 +177,21 @@ int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sa
  * instrument data and are not part of it. */
 int sim_burst_beams(sim_handle* h, const void* d_iq, int64_t n_pulses, int32_t burst, void* d_beams, uint32_t flags);
 
+/* Tabulated antenna pattern (section II.A: "all antenna patterns ... are computed and recorded on a u-v
+ * grid.  The complex values of all antenna patterns at each facet are then obtained through interpolation in the u-v
+ * grid"; reading R9).  With a table set, G(theta) of every later accumulation (fast mode;
+ * sim_regular_pulses refuses a table with SIM_ERR_BAD_CONFIG) is the complex value interpolated bilinearly at the direction cosines
+ *   u = d.e1 / R,  v = d.e2 / R,   d = r_p - r_sat,
+ *   b = unit boresight, e1 = unit vector of v_sat - (v_sat.b) b (along track, normal to b), e2 = b x e1;
+ * a direction outside [u0, u0 + (n_u-1) du] x [v0, v0 + (n_v-1) dv] is outside the recorded pattern: gain 0.
+ * d_table: DEVICE complex64 [n_v][n_u] (u fastest, interleaved re/im), 8-byte aligned, owned by the caller and kept
+ * alive while it is set; n_u, n_v in 2..4096; du, dv > 0.  d_table = NULL: back to the analytic exp(-alpha sin^2 theta).
+ * Interpolation runs in fp32: the table should resolve the pattern (relative change per cell well below 1).
+ * Errors: SIM_ERR_INVALID_ARG (sizes, steps, alignment).  An accumulation with a table set and a satellite velocity
+ * parallel to the boresight returns SIM_ERR_INVALID_ARG (no along-track axis). */
+int sim_set_antenna_lut(sim_handle* h, const void* d_table, int32_t n_u, int32_t n_v, double u0, double du, double v0,
+                        double dv);
+
 /* Runs the production index computation only: for each scatterer the gate g0 = floor(gf) in
  * [-1, G-1] and the Doppler bin k in [0, N); dropped scatterers give (SIM_GATE_NONE, -1).
  * d_gate0, d_bin: DEVICE int32[n].  Must match the canonical fp64 sequence bit for bit. */

@@ -449,6 +449,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
             float A;
             c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr, s0.v[gi + j], A);
             ab[j] = __float_as_int(A);
+            if (p.lut != nullptr) ok[j] = ok[j] && A > 0.0f;   // outside the recorded antenna pattern: contributes nothing
           }
         }
         // ---- gate, bin, weight and the guard-band test, from the two fixed-point coordinates ----
@@ -577,6 +578,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
                 if (!okj) continue;
                 float A;
                 c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], t.gfx, t.fr, s0.v[gi + j], A);
+                if (!(A > 0.0f)) continue;
               }
               global_add(p, t.g0, t.k, t.w1, c[j]);
               ++escapes;

@@ -225,19 +225,48 @@ __device__ __forceinline__ float ex2_approx(float v) {
   return r;
 }
 
-// Step A5: sqrt(s0dA) G(theta) / R^2 exp(-i 2 pi fr), all fp32.  Returns |c| in A.
-//   1/R^2 from the gate coordinate; sin^2(theta) = ((d.e1)^2 + (d.e2)^2) / R^2 with (e1, e2, boresight)
-//   orthonormal; offsets d from the satellite in fp32 (hi + lo split only where it matters: z).
+// Tabulated antenna pattern (reading R9): complex gain at the direction cosines (u, v) by bilinear
+// interpolation in p.lut [nv][nu]; false outside the recorded grid.  fp32; the four nodes come through the read-only
+// path (the table is small and shared by every scatterer: L1/L2 resident).
+__device__ __forceinline__ bool lut_gain(const AccParams& p, float u, float v, float2& g) {
+  const float fu = (u - p.lut_u0) * p.lut_inv_du, fv = (v - p.lut_v0) * p.lut_inv_dv;
+  if (!(fu >= 0.0f && fu <= (float)(p.lut_nu - 1) && fv >= 0.0f && fv <= (float)(p.lut_nv - 1))) return false;
+  const int i = min((int)fu, p.lut_nu - 2), j = min((int)fv, p.lut_nv - 2);   // the last node belongs to the last cell
+  const float a = fu - (float)i, b = fv - (float)j;
+  const float2* t = p.lut + (size_t)j * p.lut_nu + i;
+  const float2 t00 = __ldg(t), t01 = __ldg(t + 1), t10 = __ldg(t + p.lut_nu), t11 = __ldg(t + p.lut_nu + 1);
+  const float w00 = (1.0f - a) * (1.0f - b), w01 = a * (1.0f - b), w10 = (1.0f - a) * b, w11 = a * b;
+  g.x = fmaf(w11, t11.x, fmaf(w10, t10.x, fmaf(w01, t01.x, w00 * t00.x)));
+  g.y = fmaf(w11, t11.y, fmaf(w10, t10.y, fmaf(w01, t01.y, w00 * t00.y)));
+  return true;
+}
+
+// Step A5: sqrt(s0dA) G / R^2 exp(-i 2 pi fr), all fp32.  Returns an upper bound of |c| (within sqrt 2) in A.
+//   1/R^2 from the gate coordinate; offsets d from the satellite in fp32 (hi + lo split only where it matters: z);
+//   (e1, e2, boresight) orthonormal, e1 along track (reading R9): analytic gain exp(-alpha sin^2(theta)) with
+//   sin^2(theta) = ((d.e1)^2 + (d.e2)^2) / R^2, or the tabulated complex gain at (u, v) = (d.e1, d.e2) / R.
 __device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float yf, float zf, float gfx,
                                             float fr, float s0dA, float& A) {
   const float dx = xf - p.sxh, dy = yf - p.syh, dz = (zf - p.szh) - p.szl;
   const float inv_R2 = fmaf(gfx, fmaf(gfx, p.a2, p.a1), p.a0);
   const float p1 = fmaf(dz, p.e1z, fmaf(dy, p.e1y, dx * p.e1x));
   const float p2 = fmaf(dz, p.e2z, fmaf(dy, p.e2y, dx * p.e2x));
-  const float t = fmaf(p2, p2, p1 * p1);
-  A = sqrt_approx(s0dA) * ex2_approx(t * (inv_R2 * p.neg_alpha_log2e)) * inv_R2;
   float sn, cs;
   __sincosf(6.283185307179586f * fr, &sn, &cs);
+  if (p.lut != nullptr) {   // (uniform branch)
+    const float inv_R = sqrt_approx(inv_R2);
+    float2 g;
+    if (!lut_gain(p, p1 * inv_R, p2 * inv_R, g)) {
+      A = 0.0f;
+      return make_float2(0.0f, 0.0f);
+    }
+    const float A0 = sqrt_approx(s0dA) * inv_R2;
+    A = A0 * (fabsf(g.x) + fabsf(g.y));
+    const float gr = A0 * g.x, gi = A0 * g.y;
+    return make_float2(fmaf(gr, cs, gi * sn), fmaf(gi, cs, -gr * sn));   // (gr + i gi)(cs - i sn)
+  }
+  const float t = fmaf(p2, p2, p1 * p1);
+  A = sqrt_approx(s0dA) * ex2_approx(t * (inv_R2 * p.neg_alpha_log2e)) * inv_R2;
   return make_float2(A * cs, -A * sn);
 }
 

@@ -90,6 +90,10 @@ struct sim_handle {
   int opt_pt, opt_epoch;            // scatterers per lane per chunk; scatterers per fixed-point epoch
   size_t smem_per_sm;
   // stats
+  // tabulated antenna pattern (device table of the caller; nullptr: analytic gain)
+  const float2* lut;
+  int lut_nu, lut_nv;
+  double lut_u0, lut_du, lut_v0, lut_dv;
   uint64_t launches, scatterers_seen;
   bool ticket_dirty;             // the scheduling counter may be non-zero (an accumulation launch without a finalize after it)
   std::string err;
@@ -269,15 +273,23 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.syh = (float)sat->pos[1];
   p.szh = (float)sat->pos[2]; p.szl = (float)(sat->pos[2] - (double)p.szh);
   p.neg_alpha_log2e = (float)(-h->cfg.antenna_alpha * 1.4426950408889634);
-  {  // orthonormal basis (e1, e2) of the plane normal to the boresight: sin^2 = ((d.e1)^2 + (d.e2)^2) / R^2
+  {  // orthonormal basis (e1, e2) of the plane normal to the boresight: sin^2 = ((d.e1)^2 + (d.e2)^2) / R^2.
+     // e1 = along track (reading R9: the u axis of the tabulated pattern), e2 = b x e1; when the velocity is parallel
+     // to the boresight any basis serves the analytic gain (the tabulated one is refused by check_lut_frame)
     const double b[3] = {sat->boresight[0] / bn, sat->boresight[1] / bn, sat->boresight[2] / bn};
-    int ax = 0;
-    if (std::fabs(b[1]) < std::fabs(b[ax])) ax = 1;
-    if (std::fabs(b[2]) < std::fabs(b[ax])) ax = 2;
-    double a[3] = {0, 0, 0};
-    a[ax] = 1.0;
-    double e1[3] = {b[1] * a[2] - b[2] * a[1], b[2] * a[0] - b[0] * a[2], b[0] * a[1] - b[1] * a[0]};
-    const double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    const double vb = sat->vel[0] * b[0] + sat->vel[1] * b[1] + sat->vel[2] * b[2];
+    double e1[3] = {sat->vel[0] - vb * b[0], sat->vel[1] - vb * b[1], sat->vel[2] - vb * b[2]};
+    double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    const double vn = std::sqrt(sat->vel[0] * sat->vel[0] + sat->vel[1] * sat->vel[1] + sat->vel[2] * sat->vel[2]);
+    if (!(n1 > 1e-9 * vn) || !(n1 > 0)) {
+      int ax = 0;
+      if (std::fabs(b[1]) < std::fabs(b[ax])) ax = 1;
+      if (std::fabs(b[2]) < std::fabs(b[ax])) ax = 2;
+      double a[3] = {0, 0, 0};
+      a[ax] = 1.0;
+      e1[0] = b[1] * a[2] - b[2] * a[1]; e1[1] = b[2] * a[0] - b[0] * a[2]; e1[2] = b[0] * a[1] - b[1] * a[0];
+      n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    }
     for (double& v : e1) v /= n1;
     const double e2[3] = {b[1] * e1[2] - b[2] * e1[1], b[2] * e1[0] - b[0] * e1[2], b[0] * e1[1] - b[1] * e1[0]};
     p.e1x = (float)e1[0]; p.e1y = (float)e1[1]; p.e1z = (float)e1[2];
@@ -288,6 +300,11 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
     p.a2 = (float)(3.0 * dRf * dRf / (rg0 * rg0 * rg0 * rg0));
     p.w_scale = (float)(1.0 / (double)(1 << kFracBits));
   }
+  p.lut = h->lut;
+  p.lut_nu = h->lut_nu; p.lut_nv = h->lut_nv;
+  p.lut_u0 = (float)h->lut_u0; p.lut_v0 = (float)h->lut_v0;
+  p.lut_inv_du = h->lut ? (float)(1.0 / h->lut_du) : 0.0f;
+  p.lut_inv_dv = h->lut ? (float)(1.0 / h->lut_dv) : 0.0f;
   p.G = h->cfg.n_gates;
   p.N = h->cfg.n_doppler;
   p.T = T;
@@ -381,6 +398,18 @@ void scrub_accumulator(sim_handle* h) {
   cudaMemsetAsync(h->ws + h->lay.t64_off, 0, h->lay.t64_bytes, h->stream);
 }
 
+// A tabulated pattern needs its along-track axis (reading R9).
+int check_lut_frame(sim_handle* h, const sim_sat_state* sat) {
+  if (!h->lut) return SIM_OK;
+  const double bn2 = sat->boresight[0] * sat->boresight[0] + sat->boresight[1] * sat->boresight[1] + sat->boresight[2] * sat->boresight[2];
+  const double vb = sat->vel[0] * sat->boresight[0] + sat->vel[1] * sat->boresight[1] + sat->vel[2] * sat->boresight[2];
+  const double v2 = sat->vel[0] * sat->vel[0] + sat->vel[1] * sat->vel[1] + sat->vel[2] * sat->vel[2];
+  const double perp2 = v2 - vb * vb / bn2;
+  if (!(perp2 > 1e-18 * v2) || !(v2 > 0))
+    return fail(h, SIM_ERR_INVALID_ARG, "antenna table set and satellite velocity parallel to the boresight: no along-track axis");
+  return SIM_OK;
+}
+
 // Common front of the two accumulate entry points: validates everything and says which slot the update uses.
 // Changes NOTHING in the handle: the caller commits (n_updates, scatterers_seen) only after its launches succeeded.
 int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sat, uint32_t flags,
@@ -392,6 +421,8 @@ int begin_update(sim_handle* h, const sim_scatterers* s, const sim_sat_state* sa
   rc = check_sat(h, sat);
   if (rc) return rc;
   rc = check_geometry(h, sat);
+  if (rc) return rc;
+  rc = check_lut_frame(h, sat);
   if (rc) return rc;
   if (flags & SIM_ACC_APPEND) {
     if (h->n_updates == 0) return fail(h, SIM_ERR_INVALID_ARG, "SIM_ACC_APPEND before any update");
@@ -478,6 +509,9 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->stage_used[0] = h->stage_used[1] = false;
   h->n_updates = 0;
   h->pulses_emitted = 0;
+  h->lut = nullptr;
+  h->lut_nu = h->lut_nv = 0;
+  h->lut_u0 = h->lut_du = h->lut_v0 = h->lut_dv = 0.0;
   h->opt_variant = 4;
   variant_defaults(h);
   h->opt_stages = 0;
@@ -647,6 +681,7 @@ int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sa
   if (rc) return rc;
   rc = check_sat(h, sat);
   if (rc) return rc;
+  if (h->lut) return fail(h, SIM_ERR_BAD_CONFIG, "regular mode has no tabulated antenna pattern: clear the table first");
   if (n_pulses == 0) return SIM_OK;
   if (!d_iq) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer is NULL");
   if (misaligned(d_iq)) return fail(h, SIM_ERR_INVALID_ARG, "iq buffer must be 16-byte aligned");
@@ -750,6 +785,22 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   h->launches += l;
   h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
+  return SIM_OK;
+}
+
+int sim_set_antenna_lut(sim_handle* h, const void* d_table, int32_t n_u, int32_t n_v, double u0, double du, double v0, double dv) {
+  if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
+  if (!d_table) {
+    h->lut = nullptr;
+    return SIM_OK;
+  }
+  if (reinterpret_cast<uintptr_t>(d_table) & 7u) return fail(h, SIM_ERR_INVALID_ARG, "antenna table must be 8-byte aligned");
+  if (n_u < 2 || n_u > 4096 || n_v < 2 || n_v > 4096) return fail(h, SIM_ERR_INVALID_ARG, "antenna table: n_u, n_v must be in 2..4096");
+  if (!(du > 0) || !(dv > 0) || !std::isfinite(du) || !std::isfinite(dv) || !std::isfinite(u0) || !std::isfinite(v0))
+    return fail(h, SIM_ERR_INVALID_ARG, "antenna table: steps must be > 0 and origins finite");
+  h->lut = static_cast<const float2*>(d_table);
+  h->lut_nu = n_u; h->lut_nv = n_v;
+  h->lut_u0 = u0; h->lut_du = du; h->lut_v0 = v0; h->lut_dv = dv;
   return SIM_OK;
 }
 

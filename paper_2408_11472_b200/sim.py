@@ -28,7 +28,7 @@ EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",
     "sim_accumulate_update_host", "sim_synthesize_pulses_host", "sim_synchronize", "sim_destroy",
     "sim_get_spectrum", "sim_spectrum_offset", "sim_debug_indices", "sim_set_option", "sim_get_stats",
-    "sim_read_counters", "sim_last_error", "sim_regular_pulses", "sim_burst_beams",
+    "sim_read_counters", "sim_last_error", "sim_regular_pulses", "sim_burst_beams", "sim_set_antenna_lut",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library(build_if_missing: bool = True):
     L.sim_spectrum_offset.argtypes = [hp, C.c_int64, C.POINTER(C.c_size_t)]
     L.sim_debug_indices.argtypes = [hp, C.POINTER(SimScatterers), C.POINTER(SimSatState), vp, vp]
     L.sim_set_option.argtypes = [hp, C.c_int32, C.c_int64]
+    L.sim_set_antenna_lut.argtypes = [hp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double]
     L.sim_get_stats.argtypes = [hp, C.POINTER(SimStats)]
     L.sim_read_counters.argtypes = [hp, C.POINTER(C.c_uint32), C.c_int32]
     L.sim_last_error.argtypes = [hp]
@@ -245,6 +246,18 @@ class Sim:
         self._check(self.lib.sim_debug_indices(self._h, C.byref(s), C.byref(sat), g0.data_ptr() if n else None,
                                                k.data_ptr() if n else None), self._h)
         return g0, k
+
+    def set_antenna_lut(self, table: "torch.Tensor | None", u0: float = 0.0, du: float = 1.0, v0: float = 0.0,
+                        dv: float = 1.0):
+        """table: complex64 CUDA tensor [n_v][n_u] (kept alive here while it is set), or None for the analytic gain."""
+        if table is None:
+            self._lut = None
+            self._check(self.lib.sim_set_antenna_lut(self._h, None, 0, 0, 0.0, 1.0, 0.0, 1.0), self._h)
+            return
+        assert table.is_cuda and table.dtype == torch.complex64 and table.dim() == 2 and table.is_contiguous()
+        self._lut = table
+        self._check(self.lib.sim_set_antenna_lut(self._h, table.data_ptr(), table.shape[1], table.shape[0], float(u0),
+                                                 float(du), float(v0), float(dv)), self._h)
 
     def set_option(self, option: int, value: int):
         self._check(self.lib.sim_set_option(self._h, option, value), self._h)
