@@ -59,8 +59,9 @@ typedef struct sim_handle sim_handle; /* opaque, host memory, owned by the libra
 typedef struct sim_config {
   uint32_t struct_size;        /* = sizeof(sim_config); ABI guard */
   int32_t n_gates;             /* G = n_range of T_fast, 1..1024 */
-  int32_t n_doppler;           /* N = n_doppler of T_fast, power of two, 16..2048; N >= P keeps the long signals
-                                  of one segment apart (the paper's n_fast = 250..1250 run with N = 256..2048) */
+  int32_t n_doppler;           /* N = n_doppler of T_fast, 16..4096 with no prime factor other than 2, 3 and 5 (mixed-radix
+                                  inverse FFT): the paper's n_fast = 250 ... 1250 run exactly as N = P, or
+                                  as N = 2P, which keeps the past and the future half of a long signal apart (A4) */
   int32_t pulses_per_update;   /* P = n_fast, >= 1 */
   int32_t max_pending_updates; /* spectra kept in the ring, >= 2 */
   int32_t weight_mode;         /* SIM_W_SQRT (default, the paper) or SIM_W_LINEAR */

@@ -31,7 +31,7 @@ Layout make_layout(const sim_config& c) {
   L.t64_bytes = align_up((size_t)c.n_gates * c.n_doppler * sizeof(double2), 256);
   off += L.t64_bytes;
   L.tw_off = off;
-  off += align_up((size_t)(c.n_doppler / 2) * sizeof(float2), 256);
+  off += align_up((size_t)c.n_doppler * sizeof(float2), 256);
   L.ctr_off = off;
   off += align_up(kNumCounters * sizeof(unsigned int), 256);
   L.stage_off = off;
@@ -48,8 +48,11 @@ const char* check_config(const sim_config* c) {
   if (!c) return "cfg is NULL";
   if (c->struct_size != sizeof(sim_config)) return "cfg.struct_size != sizeof(sim_config) (ABI mismatch)";
   if (c->n_gates < 1 || c->n_gates > 1024) return "n_gates must be in 1..1024";
-  if (c->n_doppler < 16 || c->n_doppler > 2048 || (c->n_doppler & (c->n_doppler - 1)))
-    return "n_doppler must be a power of two in 16..2048";
+  {
+    int radix[kSynMaxPass], n_pass = 0;
+    if (c->n_doppler < 16 || c->n_doppler > 4096 || !synth_factor(c->n_doppler, radix, &n_pass))
+      return "n_doppler must be in 16..4096 with no prime factor other than 2, 3 and 5";
+  }
   if (c->pulses_per_update < 1) return "pulses_per_update must be >= 1";
   if (c->max_pending_updates < 2) return "max_pending_updates must be >= 2";
   if (c->weight_mode != SIM_W_SQRT && c->weight_mode != SIM_W_LINEAR) return "unknown weight_mode";
@@ -464,13 +467,12 @@ int do_synthesize(sim_handle* h, int64_t n_pulses, float2* d_iq, int64_t s_first
   p.n_spectra = h->n_updates;
   p.G = h->cfg.n_gates;
   p.N = h->cfg.n_doppler;
-  p.logN = 0;
-  while ((1 << p.logN) < p.N) ++p.logN;
   p.P = h->cfg.pulses_per_update;
-  p.GT = synth_gate_tile(p.N, p.G, s_last - s_first + 1, h->sm_count);
+  p.n_segments = s_last - s_first + 1;
+  synth_plan(p.N, p.G, p.n_segments, h->sm_count, &p.GT, &p.seg_per_block);
   p.weight_mode = h->cfg.weight_mode;
   int l = 0;
-  cudaError_t e = launch_synthesize(p, (int)(s_last - s_first + 1), h->stream, &l);
+  cudaError_t e = launch_synthesize(p, h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "synthesize launch");
   h->pulses_emitted += n_pulses;
@@ -549,12 +551,8 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->smem_per_sm = (size_t)v;
   e = plan_ws(h);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
-  {
-    int logN = 0;
-    while ((1 << logN) < cfg->n_doppler) ++logN;
-    e = synth_prepare(logN);
-    if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "synthesis kernel shared-memory attribute"); }
-  }
+  e = synth_prepare(cfg->n_doppler);
+  if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "synthesis kernel shared-memory attribute"); }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->ws + lay.t64_off, 0, lay.t64_bytes, h->stream);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaMemsetAsync(counters, accumulator)"); }

@@ -8,6 +8,7 @@
 namespace simk {
 
 constexpr int kNumCounters = 64;
+constexpr int kSynMaxPass = 12;                // passes of the mixed-radix inverse FFT (N <= 2048 needs at most 8)
 constexpr int kFracBits = 20;                 // fixed-point fraction bits of the gate / Doppler coordinates
 
 enum Counter : int {
@@ -76,9 +77,12 @@ struct SynParams {
   long long x0;           // first pulse of this call
   long long n_pulses;
   long long seg0;         // first segment touched
+  long long n_segments;   // segments touched by this call
   long long n_spectra;    // spectra accumulated so far (successor of s exists iff s+1 < n_spectra)
-  int G, N, logN, P;
+  int G, N, P;
   int GT;                 // gates per block
+  int seg_per_block;      // consecutive segments per block (each spectrum is transformed once per run)
+  int n_pass, radix[kSynMaxPass];   // Stockham passes: N = product of the radices (4, 2, 3, 5)
   int weight_mode;
 };
 
@@ -108,8 +112,9 @@ cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pu
 cudaError_t launch_burst_fft(const float2* Y, float2* Z, long long n_bursts, int logB, int G, cudaStream_t st,
                              int* launches);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
-cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches);
-int synth_gate_tile(int N, int G, long long n_segments, int sm_count);
-cudaError_t synth_prepare(int logN);
+cudaError_t launch_synthesize(const SynParams& p, cudaStream_t st, int* launches);
+void synth_plan(int N, int G, long long n_segments, int sm_count, int* gt, int* seg_per_block);
+bool synth_factor(int N, int* radix, int* n_pass);
+cudaError_t synth_prepare(int N);
 
 }  // namespace simk

@@ -1,21 +1,22 @@
 // Steps S1-S3: post-processing of the fast mode in one kernel.
-//   S1  batched inverse DFT along Doppler of the spectra of updates s and s+1,
-//       hand-written shared-memory FFT (decimation in frequency; radix-4 passes = two fused radix-2 stages,
-//       one radix-2 pass when log2 N is odd; natural-order load, bit-reversed read in the epilogue),
-//       unnormalised, kernel exp(+2 pi i k m / N);
+//   S1  batched inverse DFT along Doppler of the spectra: hand-written shared-memory Stockham
+//       (autosort) FFT with radix-4, -2, -3 and -5 passes, so any N = 2^a 3^b 5^c runs exactly (the paper's update
+//       intervals n_fast = 250 ... 1250, as N = P or N = 2P); unnormalised, kernel exp(+2 pi i k m / N);
 //   S2  weighting with eq. (1) and sum of the two long-time signals;
 //   S3  write of the IQ block Y[x][g], pulse-major, gate fastest.
-// One block = one segment s (pulses sP .. (s+1)P-1) x one tile of GT gates (GT a power of two).  N is a
-// template parameter: every index is a shift or a mask.
+// One block = a tile of GT gates x a run of consecutive segments: the long-time signal y_{s+1} of a segment is kept in
+// shared memory and serves as y_s of the next one, so every spectrum is transformed once per run (not twice), and the
+// IQ rows are written in pieces of GT gates (64 bytes for GT = 8).
 #include "sim_internal.h"
 
 namespace simk {
 
 constexpr int kSynThreads = 256;
 
+// tw[j] = exp(+2 pi i j / N), j < N
 __global__ void twiddle_kernel(float2* tw, int N) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j < N / 2) {
+  if (j < N) {
     double s, c;
     sincospi(2.0 * (double)j / (double)N, &s, &c);
     tw[j] = make_float2((float)c, (float)s);
@@ -23,19 +24,37 @@ __global__ void twiddle_kernel(float2* tw, int N) {
 }
 
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches) {
-  twiddle_kernel<<<(N / 2 + 127) / 128, 128, 0, st>>>(tw, N);
+  twiddle_kernel<<<(N + 127) / 128, 128, 0, st>>>(tw, N);
   ++*launches;
   return cudaGetLastError();
 }
 
-int synth_gate_tile(int N, int G, long long n_segments, int sm_count) {
-  // two signals x GT rows x (N+1) float2 (+ the twiddle table) must fit comfortably in shared memory ...
-  int gt = 16;
-  while (gt > 1 && (size_t)2 * gt * (N + 1) * sizeof(float2) > 160 * 1024) gt >>= 1;
-  // ... and the grid should give every SM several blocks: a call is a few segments x G gates, so small gate tiles
-  // are what gives it blocks.  Not below 2 gates (16-byte pieces of the gate-fastest IQ rows).
-  while (gt > 2 && n_segments * ((G + gt - 1) / gt) < 8LL * sm_count) gt >>= 1;
-  return gt;
+// N = 2^a 3^b 5^c -> passes (radix 4 first, then one 2, then 3s and 5s); false when N has another prime factor
+bool synth_factor(int N, int* radix, int* n_pass) {
+  int n = N, k = 0;
+  while (n % 4 == 0) { radix[k++] = 4; n /= 4; }
+  while (n % 2 == 0) { radix[k++] = 2; n /= 2; }
+  while (n % 3 == 0) { radix[k++] = 3; n /= 3; }
+  while (n % 5 == 0) { radix[k++] = 5; n /= 5; }
+  *n_pass = k;
+  return n == 1 && k <= kSynMaxPass;
+}
+
+size_t synth_smem_bytes(int N, int GT) { return ((size_t)3 * GT * (N + 1) + N) * sizeof(float2); }
+
+// Gates per block and segments per block.  Three signal buffers of GT rows must fit; a long call (many segments)
+// uses 8-gate tiles (64-byte IQ pieces) and runs of segments that still give about two blocks per SM; a short call
+// takes smaller tiles so that it has blocks at all.
+void synth_plan(int N, int G, long long n_segments, int sm_count, int* gt_out, int* seg_per_block) {
+  int gt = 8;
+  while (gt > 1 && synth_smem_bytes(N, gt) > 100 * 1024) gt >>= 1;
+  while (gt > 2 && n_segments * ((G + gt - 1) / gt) < sm_count / 2) gt >>= 1;
+  const long long tiles = (G + gt - 1) / gt;
+  long long runs = (2LL * sm_count + tiles - 1) / tiles;   // runs of segments wanted per gate tile
+  if (runs < 1) runs = 1;
+  if (runs > n_segments) runs = n_segments;
+  *gt_out = gt;
+  *seg_per_block = (int)((n_segments + runs - 1) / runs);
 }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -44,136 +63,188 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 cmuli(float2 a) { return make_float2(-a.y, a.x); }   // i * a
+__device__ __forceinline__ float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
 
-template <int LOGN>
+// R-point inverse DFT (kernel exp(+2 pi i a b / R)) in place
+template <int R>
+__device__ __forceinline__ void idft_small(float2* v);
+template <>
+__device__ __forceinline__ void idft_small<2>(float2* v) {
+  const float2 a = v[0], b = v[1];
+  v[0] = cadd(a, b);
+  v[1] = csub(a, b);
+}
+template <>
+__device__ __forceinline__ void idft_small<4>(float2* v) {
+  const float2 a0 = cadd(v[0], v[2]), a1 = csub(v[0], v[2]), b0 = cadd(v[1], v[3]), b1 = cmuli(csub(v[1], v[3]));
+  v[0] = cadd(a0, b0);
+  v[1] = cadd(a1, b1);
+  v[2] = csub(a0, b0);
+  v[3] = csub(a1, b1);
+}
+template <>
+__device__ __forceinline__ void idft_small<3>(float2* v) {
+  const float s3 = 0.8660254037844386f;   // sin(2 pi / 3)
+  const float2 t = cadd(v[1], v[2]), d = cscale(cmuli(csub(v[1], v[2])), s3);
+  const float2 m = make_float2(v[0].x - 0.5f * t.x, v[0].y - 0.5f * t.y);
+  v[0] = cadd(v[0], t);
+  v[1] = cadd(m, d);
+  v[2] = csub(m, d);
+}
+template <>
+__device__ __forceinline__ void idft_small<5>(float2* v) {
+  const float c1 = 0.30901699437494745f, c2 = -0.8090169943749475f;   // cos(2 pi / 5), cos(4 pi / 5)
+  const float s1 = 0.9510565162951535f, s2 = 0.5877852522924731f;     // sin(2 pi / 5), sin(4 pi / 5)
+  const float2 t1 = cadd(v[1], v[4]), t2 = cadd(v[2], v[3]), d1 = csub(v[1], v[4]), d2 = csub(v[2], v[3]);
+  const float2 m1 = make_float2(v[0].x + c1 * t1.x + c2 * t2.x, v[0].y + c1 * t1.y + c2 * t2.y);
+  const float2 m2 = make_float2(v[0].x + c2 * t1.x + c1 * t2.x, v[0].y + c2 * t1.y + c1 * t2.y);
+  const float2 e1 = cmuli(make_float2(s1 * d1.x + s2 * d2.x, s1 * d1.y + s2 * d2.y));
+  const float2 e2 = cmuli(make_float2(s2 * d1.x - s1 * d2.x, s2 * d1.y - s1 * d2.y));
+  v[0] = cadd(v[0], cadd(t1, t2));
+  v[1] = cadd(m1, e1);
+  v[4] = csub(m1, e1);
+  v[2] = cadd(m2, e2);
+  v[3] = csub(m2, e2);
+}
+
+// One Stockham pass of radix R over `rows` signals of N points: src -> dst (rows LD apart).  Ns = product of the
+// radices already done.  Butterfly j < N/R reads src[j + t N/R], twiddles by W_{Ns R}^{(j mod Ns) t}, writes
+// dst[(j - j mod Ns) R + (j mod Ns) + t Ns].
+template <int R>
+__device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, float2* __restrict__ dst, const float2* __restrict__ tw,
+                                              int rows, int N, int LD, int Ns, int tid) {
+  const int M = N / R, tstep = M / Ns;   // twiddle index k t N / (Ns R) < N: no reduction needed
+  for (int e = tid; e < rows * M; e += kSynThreads) {
+    const int row = e / M, j = e - row * M;
+    const int k = j % Ns;
+    const float2* s = src + (size_t)row * LD + j;
+    float2 v[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) v[t] = s[t * M];
+    if (Ns > 1) {
+#pragma unroll
+      for (int t = 1; t < R; ++t) v[t] = cmul(v[t], tw[k * t * tstep]);
+    }
+    idft_small<R>(v);
+    float2* d = dst + (size_t)row * LD + (j - k) * R + k;
+#pragma unroll
+    for (int t = 0; t < R; ++t) d[t * Ns] = v[t];
+  }
+}
+
 __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
-  constexpr int N = 1 << LOGN, LD = N + 1, HALF_N = N / 2;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* tw = reinterpret_cast<float2*>(smem_raw);   // [N/2] exp(+2 pi i j / N)
-  float2* sig = tw + HALF_N;                          // [2][GT][N+1]
-  const int GT = p.GT, logGT = 31 - __clz(GT);
-  const long long s = p.seg0 + blockIdx.x;
+  const int N = p.N, LD = N + 1, GT = p.GT;
+  float2* tw = reinterpret_cast<float2*>(smem_raw);   // [N] exp(+2 pi i j / N)
+  float2* buf0 = tw + N;                              // three signal buffers [GT][N+1]
+  const size_t bufsz = (size_t)GT * LD;
+  const int tid = threadIdx.x;
   const int gbase = blockIdx.y * GT;
   const int rows = min(GT, p.G - gbase);
-  const bool has_next = (s + 1 < p.n_spectra);
-  const int nsig = has_next ? 2 : 1;
-  const int tid = threadIdx.x;
+  const long long s_begin = p.seg0 + (long long)blockIdx.x * p.seg_per_block;
+  const long long s_end = min(s_begin + p.seg_per_block, p.seg0 + p.n_segments);
 
-  // ---- twiddles and spectra rows into shared memory, natural order: a straight, conflict-free copy ----
-  for (int j = tid; j < HALF_N; j += kSynThreads) tw[j] = p.tw[j];
-  for (int w = 0; w < nsig; ++w) {
-    const float2* T = p.ring + (size_t)((s + w) % p.cap) * p.slot_stride + (size_t)gbase * N;
-    float2* dst = sig + (size_t)w * GT * LD;
-    for (int e = tid; e < rows * N; e += kSynThreads) dst[(e >> LOGN) * LD + (e & (N - 1))] = T[e];
-  }
-  __syncthreads();
+  for (int j = tid; j < N; j += kSynThreads) tw[j] = p.tw[j];
 
-  // ---- S1: decimation in frequency, in place over all nsig * GT signals (rows beyond `rows` are skipped);
-  //      natural-order input, BIT-REVERSED output: y[m] ends up at index brev(m) ----
-  const int nsignals = nsig << logGT;
-  int q = LOGN;   // the next pass works inside blocks of 2^q elements
-#pragma unroll 1
-  for (; q >= 2; q -= 2) {   // stages of distance 2h and h fused (h = 2^(q-2)): elements i0 + {0, h, 2h, 3h}
-    const int h = 1 << (q - 2);
-    const int shq = LOGN - q, shh = LOGN - q + 1;   // twiddle index steps N / 4h and N / 2h
-    for (int e = tid; e < nsignals * (N / 4); e += kSynThreads) {
-      const int sidx = e >> (LOGN - 2), t = e & (N / 4 - 1);
-      if ((sidx & (GT - 1)) >= rows) continue;
-      const int j = t & (h - 1);
-      float2* x = sig + (size_t)sidx * LD + (((t >> (q - 2)) << q) + j);
-      const float2 wq = tw[j << shq], wh = tw[j << shh];
-      const float2 x0 = x[0], x1 = x[h], x2 = x[2 * h], x3 = x[3 * h];
-      const float2 a0 = cadd(x0, x2), a2 = cmul(csub(x0, x2), wq);
-      const float2 a1 = cadd(x1, x3), a3 = cmuli(cmul(csub(x1, x3), wq));   // twiddle W_4h^(j+h) = i W_4h^j
-      x[0] = cadd(a0, a1);
-      x[h] = cmul(csub(a0, a1), wh);
-      x[2 * h] = cadd(a2, a3);
-      x[3 * h] = cmul(csub(a2, a3), wh);
+  // S1 of spectrum u: rows of T_u -> buffer `a` (straight copy), passes between `a` and `b`; returns where y_u ended up
+  auto transform = [&](long long u, float2* a, float2* b) -> float2* {
+    const float2* T = p.ring + (size_t)(u % p.cap) * p.slot_stride + (size_t)gbase * N;
+    for (int e = tid; e < rows * N; e += kSynThreads) {
+      const int row = e / N;
+      a[(size_t)row * LD + (e - row * N)] = T[e];
     }
     __syncthreads();
-  }
-  if (q == 1) {  // log2 N odd: the last stage (distance 1, twiddle 1) on its own
-    for (int e = tid; e < nsignals * HALF_N; e += kSynThreads) {
-      const int sidx = e >> (LOGN - 1), t = e & (HALF_N - 1);
-      if ((sidx & (GT - 1)) >= rows) continue;
-      float2* x = sig + (size_t)sidx * LD + 2 * t;
-      const float2 a = x[0], b = x[1];
-      x[0] = cadd(a, b);
-      x[1] = csub(a, b);
+    int Ns = 1;
+    for (int ps = 0; ps < p.n_pass; ++ps) {
+      const int R = p.radix[ps];
+      if (R == 4) stockham_pass<4>(a, b, tw, rows, N, LD, Ns, tid);
+      else if (R == 2) stockham_pass<2>(a, b, tw, rows, N, LD, Ns, tid);
+      else if (R == 3) stockham_pass<3>(a, b, tw, rows, N, LD, Ns, tid);
+      else stockham_pass<5>(a, b, tw, rows, N, LD, Ns, tid);
+      __syncthreads();
+      Ns *= R;
+      float2* t = a; a = b; b = t;
     }
-    __syncthreads();
-  }
+    return a;
+  };
 
-  // ---- S2 + S3: cross-fade and write, gate fastest ----
-  const long long seg_lo = s * (long long)p.P;
-  const long long lo = max(seg_lo, p.x0), hi = min(seg_lo + p.P, p.x0 + p.n_pulses);
-  const int npul = (int)(hi - lo);
+  float2* cur = buf0;
+  float2* f1 = buf0 + bufsz;
+  float2* f2 = buf0 + 2 * bufsz;
+  {
+    float2* r = transform(s_begin, cur, f1);
+    if (r != cur) { f1 = cur; cur = r; }
+  }
   const float invP = 1.0f / (float)p.P;
-  for (int e = tid; e < (npul << logGT); e += kSynThreads) {
-    const int pi = e >> logGT, row = e & (GT - 1);
-    if (row >= rows) continue;
-    const long long x = lo + pi;
-    const int m = (int)(x - seg_lo);  // 0..P-1
-    const float2 ys = sig[(size_t)row * LD + (int)(__brev((unsigned)(m & (N - 1))) >> (32 - LOGN))];
-    float2 out;
+  const int P = p.P;
+  for (long long s = s_begin; s < s_end; ++s) {
+    const bool has_next = (s + 1 < p.n_spectra);
+    float2* nxt = nullptr;
     if (has_next) {
-      const float a = (float)m * invP;
-      float ws = 1.0f - a, wn = a;
-      if (p.weight_mode == SIM_W_SQRT) {
-        ws = sqrtf(ws);
-        wn = sqrtf(wn);
-      }
-      const float2 yn = sig[((size_t)GT + row) * LD + (int)(__brev((unsigned)((m - p.P) & (N - 1))) >> (32 - LOGN))];
-      out = make_float2(ws * ys.x + wn * yn.x, ws * ys.y + wn * yn.y);
-    } else {
-      out = ys;  // tail rule: lone spectrum at weight 1
+      nxt = transform(s + 1, f1, f2);
+      if (nxt != f1) { f2 = f1; f1 = nxt; }   // (f1 now names the buffer holding y_{s+1}; f2 the free one)
     }
-    p.iq[(size_t)(x - p.x0) * p.G + gbase + row] = out;
+    // ---- S2 + S3: cross-fade and write, gate fastest ----
+    const long long seg_lo = s * (long long)P;
+    const long long lo = max(seg_lo, p.x0), hi = min(seg_lo + P, p.x0 + p.n_pulses);
+    const int npul = (int)(hi - lo);
+    for (int e = tid; e < npul * GT; e += kSynThreads) {
+      const int pi = e / GT, row = e - pi * GT;
+      if (row >= rows) continue;
+      const long long x = lo + pi;
+      const int m = (int)(x - seg_lo);  // 0..P-1
+      const float2 ys = cur[(size_t)row * LD + (m % N)];
+      float2 out;
+      if (has_next) {
+        const float a = (float)m * invP;
+        float ws = 1.0f - a, wn = a;
+        if (p.weight_mode == SIM_W_SQRT) {
+          ws = sqrtf(ws);
+          wn = sqrtf(wn);
+        }
+        int mn = (m - P) % N;           // in (-N, 0]
+        mn += mn < 0 ? N : 0;
+        const float2 yn = nxt[(size_t)row * LD + mn];
+        out = make_float2(ws * ys.x + wn * yn.x, ws * ys.y + wn * yn.y);
+      } else {
+        out = ys;  // tail rule: lone spectrum at weight 1
+      }
+      p.iq[(size_t)(x - p.x0) * p.G + gbase + row] = out;
+    }
+    __syncthreads();   // the emission has read `cur`: it becomes a free buffer
+    if (has_next) {
+      float2* t = cur; cur = f1; f1 = t;
+    }
   }
 }
 
-typedef void (*SynKernel)(SynParams);
-
-static SynKernel syn_kernel(int logN) {
-  switch (logN) {
-    case 4: return synth_kernel<4>;
-    case 5: return synth_kernel<5>;
-    case 6: return synth_kernel<6>;
-    case 7: return synth_kernel<7>;
-    case 8: return synth_kernel<8>;
-    case 9: return synth_kernel<9>;
-    case 10: return synth_kernel<10>;
-    case 11: return synth_kernel<11>;
-    default: return nullptr;
-  }
+// Once per handle: the dynamic shared-memory limit of the kernel (largest plan for this N).
+cudaError_t synth_prepare(int N) {
+  int gt = 8;
+  while (gt > 1 && synth_smem_bytes(N, gt) > 100 * 1024) gt >>= 1;
+  return cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synth_smem_bytes(N, gt));
 }
 
-size_t synth_smem_bytes(int N, int GT) { return ((size_t)2 * GT * (N + 1) + N / 2) * sizeof(float2); }
-
-// Once per handle: the dynamic shared-memory limit of the kernel for this N (largest gate tile).
-cudaError_t synth_prepare(int logN) {
-  SynKernel k = syn_kernel(logN);
-  if (!k) return cudaErrorInvalidValue;
-  const int N = 1 << logN;
-  return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)synth_smem_bytes(N, synth_gate_tile(N, 1, 1 << 30, 1)));
-}
-
-cudaError_t launch_synthesize(const SynParams& p, int n_segments, cudaStream_t st, int* launches) {
-  if (n_segments <= 0 || p.n_pulses <= 0) return cudaSuccess;
-  SynKernel k = syn_kernel(p.logN);
-  if (!k) return cudaErrorInvalidValue;
+cudaError_t launch_synthesize(const SynParams& p0, cudaStream_t st, int* launches) {
+  if (p0.n_segments <= 0 || p0.n_pulses <= 0) return cudaSuccess;
+  SynParams p = p0;
+  if (!synth_factor(p.N, p.radix, &p.n_pass)) return cudaErrorInvalidValue;
   const size_t smem = synth_smem_bytes(p.N, p.GT);
-  // gridDim.x (segments) can be large for long tracks; gridDim.y (gate tiles) <= 1024
+  // per launch: the limit is per function and per device, another handle may have set it for a smaller N
+  cudaError_t e = cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
   const int gy = (p.G + p.GT - 1) / p.GT;
-  int done = 0;
-  while (done < n_segments) {
-    const int nx = (n_segments - done) < 65535 * 32 ? (n_segments - done) : 65535 * 32;
+  const long long runs = (p.n_segments + p.seg_per_block - 1) / p.seg_per_block;
+  long long done = 0;
+  while (done < runs) {   // gridDim.x can be large for long tracks
+    const long long nx = (runs - done) < (1LL << 30) ? (runs - done) : (1LL << 30);
     SynParams q = p;
-    q.seg0 = p.seg0 + done;
-    k<<<dim3(nx, gy), kSynThreads, smem, st>>>(q);
+    q.seg0 = p.seg0 + done * p.seg_per_block;
+    q.n_segments = p.n_segments - done * p.seg_per_block;
+    if (q.n_segments > nx * p.seg_per_block) q.n_segments = nx * p.seg_per_block;
+    synth_kernel<<<dim3((unsigned)nx, gy), kSynThreads, smem, st>>>(q);
     ++*launches;
-    const cudaError_t e = cudaGetLastError();
+    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     done += nx;
   }

@@ -514,11 +514,15 @@ def test_regular_mode_errors(sim_mod):
 
 
 # ---- the paper's own sizes (n_fast = 250 ... 1250; PAPER.md:73 fence-post) ----
-@pytest.mark.parametrize("P,N", [(250, 256), (500, 512), (1000, 1024), (1250, 2048)])
+PAPER_SIZES = [(P, f * P) for P in (250, 500, 750, 1000, 1250) for f in (1, 2)] + [(250, 256), (1250, 2048), (750, 1024)]
+
+
+@pytest.mark.parametrize("P,N", PAPER_SIZES)
 def test_paper_shaped_update_intervals(oracle, sim_mod, P, N):
-    """n_fast is not a power of two in the paper: the Doppler axis takes the next power of two (the long signal of
-    an update then covers its two segments without wrapping onto itself), and the track is synthesised the paper's
-    way: 1 + n_pulses / n_fast spectra, every segment bracketed by two of them (no tail rule)."""
+    """n_fast is not a power of two in the paper (250 ... 1250 by 250): the Doppler axis runs EXACTLY at N = n_fast and
+    at N = 2 n_fast (mixed-radix inverse FFT, N = 2^a 3^b 5^c), and also padded to a power of two; the track is
+    synthesised the paper's way: 1 + n_pulses / n_fast spectra, every segment bracketed by two of them (no tail rule).
+    Spectra, IQ blocks (<= 1e-4) and all bin indices (bit-exact; bins are taken mod N, any N)."""
     wl = W.get("nadir_patch_16m").scaled(n_along=200, n_cross=256, n_doppler=N, pulses_per_update=P, n_updates=4)
     scat = W.scatterers(wl)
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
@@ -527,6 +531,7 @@ def test_paper_shaped_update_intervals(oracle, sim_mod, P, N):
     for u in range(wl.n_updates):
         sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, u))
         assert U.rel_l2(sim.get_spectrum(u).cpu().numpy(), T_ref[u]) <= U.TOL
+    _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=wl.n_updates - 1)
     n = (wl.n_updates - 1) * P                                   # whole-track batch post-processing, no SYN_FINAL
     iq = sim.synthesize_pulses(n).cpu().numpy()
     Y = oracle.synthesize(U.oracle_cfg(oracle, wl), T_ref, 0, n, final=False)
