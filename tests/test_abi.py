@@ -51,7 +51,7 @@ def test_workspace_bytes_and_config_validation(sim_mod):
                                host_stage_scatterers=1 << 20, host_stage_pulses=2048)
     assert lib.sim_workspace_bytes(C.byref(cfg2), C.byref(n)) == sim_mod.OK
     assert n.value >= base + 2 * 7 * 4 * (1 << 20) + 2048 * 128 * 8
-    bad = [dict(n_doppler=100), dict(n_doppler=8), dict(n_doppler=4096), dict(n_gates=0), dict(n_gates=1025),
+    bad = [dict(n_doppler=112), dict(n_doppler=8), dict(n_doppler=4098), dict(n_doppler=8192), dict(n_gates=0), dict(n_gates=1025),
            dict(pulses_per_update=0), dict(max_pending_updates=1), dict(weight_mode=7), dict(wavelength_m=0.0),
            dict(prf_hz=-1.0), dict(gate_spacing_m=float("nan")), dict(antenna_alpha=-1.0),
            dict(host_stage_scatterers=3)]
