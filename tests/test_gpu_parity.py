@@ -372,13 +372,13 @@ def test_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
 
 def test_coherent_pileup_cannot_overflow(oracle, sim_mod):
     """Worst case for the int32 tiles: every scatterer of a long epoch lands in the SAME cell with the SAME
-    phase (identical positions and velocities), amplitudes up to just below the admitted maximum.  (Escapes are
-    kept out of this case on purpose: 10^5 identical fp32 increments added one by one to the same global cell
-    lose their low bits systematically, which is a property of fp32 accumulation, not of the tiles.)"""
+    phase (identical positions and velocities).  Amplitude ratios up to 3.9 x the epoch's geometric mean: the
+    brightest leave the admitted fixed-point range and take the escape path, whose global accumulator is fp64
+    (10^5 identical increments into one cell lose nothing), so the bound holds for them too."""
     wl = W.get("tiny").scaled(n_updates=1)
     n = 300_000
     g = torch.Generator().manual_seed(7)
-    ratio = torch.tensor([1.0, 1.4, 0.6, 0.35])[torch.randint(0, 4, (n,), generator=g)]   # max / gmean < 2: all admitted
+    ratio = torch.tensor([1.0, 1.9, 3.9, 0.6, 0.35])[torch.randint(0, 5, (n,), generator=g)]
     scat = {"x": torch.zeros(n), "y": torch.zeros(n), "z": torch.full((n,), 0.1), "vx": torch.zeros(n),
             "vy": torch.zeros(n), "vz": torch.zeros(n), "s0dA": 10.0 * ratio * ratio}
     scat = {k: v.float().contiguous() for k, v in scat.items()}
@@ -392,7 +392,6 @@ def test_coherent_pileup_cannot_overflow(oracle, sim_mod):
         sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
         e = U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref)
         assert e <= U.TOL, (variant, epoch, e)
-        assert sim.read_counters()["escapes"] == 0
 
 
 # ---- the paper's pulse-pair Doppler (Algorithm 1 lines 5-7) --------
