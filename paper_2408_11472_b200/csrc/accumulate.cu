@@ -168,7 +168,7 @@ __device__ __forceinline__ void global_add(const AccParams& p, int g0, int k, fl
   }
 }
 
-template <int NCW, int PT, int IL, int MODE, bool DBG>
+template <int NCW, int PT, int IL, int MODE, bool DBG, bool LUT>
 __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccParams p) {
   constexpr int CH = NCW * 32 * PT, SL = 32 * PT;
   constexpr unsigned kStageBytes = 7u * CH * 4u;
@@ -447,9 +447,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   #pragma unroll
           for (int j = 0; j < IL; ++j) {
             float A;
-            c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr, s0.v[gi + j], A);
+            c[j] = amplitude_t<LUT>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr, s0.v[gi + j], A);
             ab[j] = __float_as_int(A);
-            if (p.lut != nullptr) ok[j] = ok[j] && A > 0.0f;   // outside the recorded antenna pattern: contributes nothing
+            if (LUT) ok[j] = ok[j] && A > 0.0f;   // outside the recorded antenna pattern: contributes nothing
           }
         }
         // ---- gate, bin, weight and the guard-band test, from the two fixed-point coordinates ----
@@ -577,7 +577,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
                                            __dsub_rn((double)z.v[gi + j], p.sz), vx.v[gi + j], vy.v[gi + j], vz.v[gi + j], t);
                 if (!okj) continue;
                 float A;
-                c[j] = amplitude(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], t.gfx, t.fr, s0.v[gi + j], A);
+                c[j] = amplitude_t<LUT>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], t.gfx, t.fr, s0.v[gi + j], A);
                 if (!(A > 0.0f)) continue;
               }
               global_add(p, t.g0, t.k, t.w1, c[j]);
@@ -665,29 +665,30 @@ int acc_index_mode(const AccParams& p) {
 // ---------------------------------------------------------------------------------------------
 typedef void (*AccKernel)(AccParams);
 
-static AccKernel acc_kernel_ptr(int ncw, int pt, int il, int mode, bool dbg) {
-#define ACC_CASE(NCW_, PT_, IL_)                                                                       \
-  if (ncw == NCW_ && pt == PT_ && il == IL_) {                                                         \
-    if (dbg)                                                                                           \
-      return mode == kIdxFast ? acc_kernel<NCW_, PT_, IL_, kIdxFast, true>                             \
-           : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, true>           \
-                                       : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, true>;              \
-    return mode == kIdxFast ? acc_kernel<NCW_, PT_, IL_, kIdxFast, false>                              \
-         : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, false>            \
-                                     : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, false>;               \
-  }
+// kind: 0 accumulate with the analytic gain, 1 accumulate with the tabulated gain, 2 index export
+static AccKernel acc_kernel_ptr(int ncw, int pt, int il, int mode, int kind) {
+#define ACC_MODE(NCW_, PT_, IL_, DBG_, LUT_)                                                                   \
+  (mode == kIdxFast ? acc_kernel<NCW_, PT_, IL_, kIdxFast, DBG_, LUT_>                                         \
+   : mode == kIdxFastPulsePair ? acc_kernel<NCW_, PT_, IL_, kIdxFastPulsePair, DBG_, LUT_>                     \
+                               : acc_kernel<NCW_, PT_, IL_, kIdxCanonical, DBG_, LUT_>)
+#define ACC_CASE(NCW_, PT_, IL_)                                                                               \
+  if (ncw == NCW_ && pt == PT_ && il == IL_)                                                                   \
+    return kind == 2 ? ACC_MODE(NCW_, PT_, IL_, true, false) : kind == 1 ? ACC_MODE(NCW_, PT_, IL_, false, true) \
+                                                                         : ACC_MODE(NCW_, PT_, IL_, false, false);
   ACC_CASE(8, 4, 4) ACC_CASE(8, 4, 2) ACC_CASE(8, 2, 2) ACC_CASE(16, 4, 4)
 #undef ACC_CASE
+#undef ACC_MODE
   return nullptr;
 }
 
-bool acc_supported(int ncw, int pt, int il) { return acc_kernel_ptr(ncw, pt, il, kIdxFast, false) != nullptr; }
+bool acc_supported(int ncw, int pt, int il) { return acc_kernel_ptr(ncw, pt, il, kIdxFast, 0) != nullptr; }
 
 cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks) {
   const size_t smem = acc_smem_bytes(G, W, ncw, pt, stages);
   *blocks = 1 << 30;
-  for (int mode = 0; mode < 3; ++mode) {
-    AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, false);
+  for (int mk = 0; mk < 6; ++mk) {
+    const int mode = mk % 3;
+    AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, mk / 3);
     if (!k) return cudaErrorInvalidValue;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -704,7 +705,7 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
                               int* launches) {
   if (p.n == 0) return cudaSuccess;
   const int mode = acc_index_mode(p);
-  AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, dbg);
+  AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, dbg ? 2 : (p.lut != nullptr ? 1 : 0));
   if (!k) return cudaErrorInvalidValue;
   const size_t smem = acc_smem_bytes(p.G, p.W, ncw, pt, p.stages);
   // per launch: the limit is per function and per device, another handle may have set it for a smaller shape

@@ -245,15 +245,16 @@ __device__ __forceinline__ bool lut_gain(const AccParams& p, float u, float v, f
 //   1/R^2 from the gate coordinate; offsets d from the satellite in fp32 (hi + lo split only where it matters: z);
 //   (e1, e2, boresight) orthonormal, e1 along track (reading R9): analytic gain exp(-alpha sin^2(theta)) with
 //   sin^2(theta) = ((d.e1)^2 + (d.e2)^2) / R^2, or the tabulated complex gain at (u, v) = (d.e1, d.e2) / R.
-__device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float yf, float zf, float gfx,
-                                            float fr, float s0dA, float& A) {
+template <bool LUT>
+__device__ __forceinline__ float2 amplitude_t(const AccParams& p, float xf, float yf, float zf, float gfx,
+                                              float fr, float s0dA, float& A) {
   const float dx = xf - p.sxh, dy = yf - p.syh, dz = (zf - p.szh) - p.szl;
   const float inv_R2 = fmaf(gfx, fmaf(gfx, p.a2, p.a1), p.a0);
   const float p1 = fmaf(dz, p.e1z, fmaf(dy, p.e1y, dx * p.e1x));
   const float p2 = fmaf(dz, p.e2z, fmaf(dy, p.e2y, dx * p.e2x));
   float sn, cs;
   __sincosf(6.283185307179586f * fr, &sn, &cs);
-  if (p.lut != nullptr) {   // (uniform branch)
+  if (LUT) {
     const float inv_R = sqrt_approx(inv_R2);
     float2 g;
     if (!lut_gain(p, p1 * inv_R, p2 * inv_R, g)) {
@@ -268,6 +269,11 @@ __device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float 
   const float t = fmaf(p2, p2, p1 * p1);
   A = sqrt_approx(s0dA) * ex2_approx(t * (inv_R2 * p.neg_alpha_log2e)) * inv_R2;
   return make_float2(A * cs, -A * sn);
+}
+// run-time choice (kernels off the hot path: reference, regular mode)
+__device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float yf, float zf, float gfx, float fr,
+                                            float s0dA, float& A) {
+  return p.lut != nullptr ? amplitude_t<true>(p, xf, yf, zf, gfx, fr, s0dA, A) : amplitude_t<false>(p, xf, yf, zf, gfx, fr, s0dA, A);
 }
 
 }  // namespace simk
