@@ -109,14 +109,15 @@ __device__ __forceinline__ void idft_small<5>(float2* v) {
 
 // One Stockham pass of radix R over `rows` signals of N points: src -> dst (rows LD apart).  Ns = product of the
 // radices already done.  Butterfly j < N/R reads src[j + t N/R], twiddles by W_{Ns R}^{(j mod Ns) t}, writes
-// dst[(j - j mod Ns) R + (j mod Ns) + t Ns].
-template <int R>
+// dst[(j - j mod Ns) R + (j mod Ns) + t Ns].  POW2: N/R and Ns are powers of two (every index is a shift or a mask).
+template <int R, bool POW2>
 __device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, float2* __restrict__ dst, const float2* __restrict__ tw,
                                               int rows, int N, int LD, int Ns, int tid) {
   const int M = N / R, tstep = M / Ns;   // twiddle index k t N / (Ns R) < N: no reduction needed
+  const int logM = 31 - __clz(M);
   for (int e = tid; e < rows * M; e += kSynThreads) {
-    const int row = e / M, j = e - row * M;
-    const int k = j % Ns;
+    const int row = POW2 ? (e >> logM) : (e / M), j = POW2 ? (e & (M - 1)) : (e - row * M);
+    const int k = POW2 ? (j & (Ns - 1)) : (j % Ns);
     const float2* s = src + (size_t)row * LD + j;
     float2 v[R];
 #pragma unroll
@@ -146,21 +147,31 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
 
   for (int j = tid; j < N; j += kSynThreads) tw[j] = p.tw[j];
 
+  const bool pow2 = (N & (N - 1)) == 0;
+  const int logN = 31 - __clz(N), logGT = 31 - __clz(GT);
   // S1 of spectrum u: rows of T_u -> buffer `a` (straight copy), passes between `a` and `b`; returns where y_u ended up
   auto transform = [&](long long u, float2* a, float2* b) -> float2* {
     const float2* T = p.ring + (size_t)(u % p.cap) * p.slot_stride + (size_t)gbase * N;
-    for (int e = tid; e < rows * N; e += kSynThreads) {
-      const int row = e / N;
-      a[(size_t)row * LD + (e - row * N)] = T[e];
+    if (pow2) {
+#pragma unroll 4
+      for (int e = tid; e < rows * N; e += kSynThreads) a[(size_t)(e >> logN) * LD + (e & (N - 1))] = T[e];
+    } else {
+      for (int row = 0; row < rows; ++row)
+        for (int j = tid; j < N; j += kSynThreads) a[(size_t)row * LD + j] = T[(size_t)row * N + j];
     }
     __syncthreads();
     int Ns = 1;
     for (int ps = 0; ps < p.n_pass; ++ps) {
       const int R = p.radix[ps];
-      if (R == 4) stockham_pass<4>(a, b, tw, rows, N, LD, Ns, tid);
-      else if (R == 2) stockham_pass<2>(a, b, tw, rows, N, LD, Ns, tid);
-      else if (R == 3) stockham_pass<3>(a, b, tw, rows, N, LD, Ns, tid);
-      else stockham_pass<5>(a, b, tw, rows, N, LD, Ns, tid);
+      if (pow2) {
+        if (R == 4) stockham_pass<4, true>(a, b, tw, rows, N, LD, Ns, tid);
+        else stockham_pass<2, true>(a, b, tw, rows, N, LD, Ns, tid);
+      } else {
+        if (R == 4) stockham_pass<4, false>(a, b, tw, rows, N, LD, Ns, tid);
+        else if (R == 2) stockham_pass<2, false>(a, b, tw, rows, N, LD, Ns, tid);
+        else if (R == 3) stockham_pass<3, false>(a, b, tw, rows, N, LD, Ns, tid);
+        else stockham_pass<5, false>(a, b, tw, rows, N, LD, Ns, tid);
+      }
       __syncthreads();
       Ns *= R;
       float2* t = a; a = b; b = t;
@@ -188,12 +199,16 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
     const long long seg_lo = s * (long long)P;
     const long long lo = max(seg_lo, p.x0), hi = min(seg_lo + P, p.x0 + p.n_pulses);
     const int npul = (int)(hi - lo);
-    for (int e = tid; e < npul * GT; e += kSynThreads) {
-      const int pi = e / GT, row = e - pi * GT;
+    int off_n = (-P) % N;            // (m - P) mod N = (m + off_n) mod N, off_n in [0, N)
+    off_n += off_n < 0 ? N : 0;
+    for (int e = tid; e < (npul << logGT); e += kSynThreads) {
+      const int pi = e >> logGT, row = e & (GT - 1);
       if (row >= rows) continue;
       const long long x = lo + pi;
       const int m = (int)(x - seg_lo);  // 0..P-1
-      const float2 ys = cur[(size_t)row * LD + (m % N)];
+      int ms = m;
+      while (ms >= N) ms -= N;          // P / N turns at most
+      const float2 ys = cur[(size_t)row * LD + ms];
       float2 out;
       if (has_next) {
         const float a = (float)m * invP;
@@ -202,8 +217,8 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
           ws = sqrtf(ws);
           wn = sqrtf(wn);
         }
-        int mn = (m - P) % N;           // in (-N, 0]
-        mn += mn < 0 ? N : 0;
+        int mn = ms + off_n;
+        mn -= mn >= N ? N : 0;
         const float2 yn = nxt[(size_t)row * LD + mn];
         out = make_float2(ws * ys.x + wn * yn.x, ws * ys.y + wn * yn.y);
       } else {
