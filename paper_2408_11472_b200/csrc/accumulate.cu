@@ -178,10 +178,10 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   __shared__ int s_useq[kRing];
   __shared__ int s_claimed;             // units that some warp has entered (the first one in prepares unit + 2)
   __shared__ int s_slot[4][kSlotInts];
-  __shared__ int s_tcount[2];           // warps that have finished the running epoch of tile b
-  __shared__ int s_complete[2];         // epochs of tile b that every warp has finished
+  // per tile b, one phase per epoch that uses it (NCW arrivals each): "every warp has finished the epoch" and "every warp
+  // has drained its share of it".  Waiters sleep in hardware (try_wait with a suspend hint) instead of spinning.
+  __shared__ __align__(8) unsigned long long s_bar_complete[2], s_bar_drained[2];
   __shared__ int s_shares[2];           // warps that have drained their share of the completed epoch of tile b
-  __shared__ int s_drained[2];          // epochs of tile b drained by every warp
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int S = p.stages, EC = p.epoch_chunks;
@@ -191,8 +191,8 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   const unsigned plane_bytes = (unsigned)p.plane_words * 4u, tile_bytes = 4u * plane_bytes;
   const UnitTable ut{sh::addr(&s_ustart[0]), sh::addr(&s_uend[0]), sh::addr(&s_useq[0])};
   const unsigned claimed_a = sh::addr(&s_claimed);
-  const unsigned tcount0 = sh::addr(&s_tcount[0]), drained0 = sh::addr(&s_drained[0]);
-  const unsigned complete0 = sh::addr(&s_complete[0]), shares0 = sh::addr(&s_shares[0]);
+  const unsigned complete0 = sh::addr(&s_bar_complete[0]), drained0 = sh::addr(&s_bar_drained[0]);
+  const unsigned shares0 = sh::addr(&s_shares[0]);
   const unsigned slot0 = sh::addr(&s_slot[0][0]);
   const unsigned cps = (unsigned)(p.superchunk / CH);          // chunks per scheduling unit
   // the copies run one chunk ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
@@ -208,10 +208,10 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   for (int i = tid; i < kRing; i += NCW * 32) sh::st(ut.seq0 + 4u * i, 0);
   if (tid < 4) sh::st(slot0 + 4u * kSlotInts * tid + 4 * kSlotState, kSlotUnset);
   if (tid < 2) {
-    sh::st(tcount0 + 4u * tid, 0);
-    sh::st(drained0 + 4u * tid, 0);
-    sh::st(complete0 + 4u * tid, 0);
+    sh::mbar_init(complete0 + 8u * tid, NCW);
+    sh::mbar_init(drained0 + 8u * tid, NCW);
     sh::st(shares0 + 4u * tid, 0);
+    sh::mbar_fence_init();
   }
   __syncthreads();
   if (tid == 0) {   // the first `ahead` units
@@ -311,10 +311,12 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       }
     }
     __syncwarp();
-    if (lane == 0 && sh::atom_add_acq_rel(shares0 + 4u * b, 1) == NCW - 1) {   // every share is out: tile and slot go back
-      sh::st(shares0 + 4u * b, 0);
-      sh::st(slot + 4 * kSlotState, kSlotUnset);
-      sh::st_release(drained0 + 4u * b, (int)(d >> 1) + 1);
+    if (lane == 0) {
+      if (sh::atom_add_acq_rel(shares0 + 4u * b, 1) == NCW - 1) {   // every share is out: the slot goes back ...
+        sh::st(shares0 + 4u * b, 0);
+        sh::st(slot + 4 * kSlotState, kSlotUnset);
+      }
+      sh::mbar_arrive(drained0 + 8u * b);                             // ... and, with the last arrival, the tile
     }
     __syncwarp();
   };
@@ -324,11 +326,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   auto try_drain = [&](unsigned upto, bool block) {
     while (dpend < upto) {
       const unsigned b = dpend & 1u;
-      if (sh::ld_acquire(complete0 + 4u * b) <= (int)(dpend >> 1)) {
-        if (!block) return;
-        __nanosleep(256);   // a warp that is ahead must not take issue slots from the ones it waits for
-        continue;
-      }
+      const unsigned par = (dpend >> 1) & 1u;
+      if (block) sh::mbar_wait_sleepy(complete0 + 8u * b, par, 2000u);   // a warp that is ahead sleeps: no issue slots taken
+      else if (!sh::mbar_test(complete0 + 8u * b, par)) return;
       drain_share(dpend);
       ++dpend;
     }
@@ -349,7 +349,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     const unsigned slot = slot0 + 4u * kSlotInts * (e & 3u);
     if (!DBG && e >= 2) {   // the tile of epoch e-2 must be back: this warp's own share first, then everybody else's
       try_drain(e - 1u, true);
-      while (sh::ld_acquire(drained0 + 4u * (e & 1u)) < (int)(e >> 1)) __nanosleep(256);
+      sh::mbar_wait_sleepy(drained0 + 8u * (e & 1u), ((e >> 1) - 1u) & 1u, 2000u);
     }
     // tile base of this lane's first reduction, the +1 row offset of the padded tile folded in
     const unsigned tile_b = tile0 + (e & 1u) * tile_bytes + (unsigned)RS4 + off_b0;
@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     float s = 0.0f, sS = 0.0f, sO = 0.0f;
     int ci = 0;
     for (; ci < EC; ++ci) {
-      if (!DBG && dpend < e && sh::ld_acquire(complete0 + 4u * (dpend & 1u)) > (int)(dpend >> 1)) try_drain(e, false);
+      if (!DBG && dpend < e && sh::mbar_test(complete0 + 8u * (dpend & 1u), (dpend >> 1) & 1u)) try_drain(e, false);
       // the next chunk goes into the stage that was read one iteration ago; then this lane's copies of the chunk to read
       // (one group older) must have landed
       copy_chunk(stg ^ 1u);
@@ -595,10 +595,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     // ---- end of an epoch (or of the input inside one): the last warp out declares the tile complete ----
     if (!DBG) {
       __syncwarp();
-      if (lane == 0 && sh::atom_add_acq_rel(tcount0 + 4u * (e & 1u), 1) == NCW - 1) {
-        sh::st(tcount0 + 4u * (e & 1u), 0);
-        sh::st_release(complete0 + 4u * (e & 1u), (int)(e >> 1) + 1);
-      }
+      if (lane == 0) sh::mbar_arrive(complete0 + 8u * (e & 1u));   // the last warp out completes the phase: the tile can be drained
       __syncwarp();
       if (!more) try_drain(e + 1u, true);   // the end of the input: the shares of the last epochs
     }

@@ -115,6 +115,18 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity, uns
       : "memory");
   return ok != 0;
 }
+// One non-blocking test: has the phase of parity `parity` completed?
+__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity) {
+  unsigned ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait_sleepy(unsigned bar, unsigned parity, unsigned hint_ns) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
