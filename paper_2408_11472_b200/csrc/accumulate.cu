@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
             // g0 and a 20-bit weight for the tile path; the bin itself (no fraction bits)
             fx[j].gfx = (cx[j].g0 << kFracBits) + min((int)(cx[j].w1 * (float)kFxOne), kFxOne - 1);
             fx[j].kfx = cx[j].k;
-            fx[j].fr = cx[j].fr;
+            fx[j].fr = cx[j].fr * 4294967296.0f;   // cycles -> units of 2^-32 cycles
           }
         } else {
           // polynomial path straight through for all IL scatterers; the guard-band cases are re-decided in the cold block
@@ -444,12 +444,26 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
             fx[j] = index_fx<MODE>(p, q[j], x.v[gi + j], y.v[gi + j], z.v[gi + j], vx.v[gi + j], vy.v[gi + j], vz.v[gi + j]);
         }
         if (!DBG) {
+          if (LUT) {
   #pragma unroll
-          for (int j = 0; j < IL; ++j) {
-            float A;
-            c[j] = amplitude_t<LUT>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr, s0.v[gi + j], A);
-            ab[j] = __float_as_int(A);
-            if (LUT) ok[j] = ok[j] && A > 0.0f;   // outside the recorded antenna pattern: contributes nothing
+            for (int j = 0; j < IL; ++j) {
+              float A;
+              c[j] = amplitude_t<true>(p, x.v[gi + j], y.v[gi + j], z.v[gi + j], (float)fx[j].gfx, fx[j].fr * kFrUnit, s0.v[gi + j], A);
+              ab[j] = __float_as_int(A);
+              ok[j] = ok[j] && A > 0.0f;   // outside the recorded antenna pattern: contributes nothing
+            }
+          } else {   // two scatterers per packed fp32 instruction
+  #pragma unroll
+            for (int j = 0; j < IL; j += 2) {
+              float2 A, cre, cim;
+              amplitude_pair(p, make_float2(x.v[gi + j], x.v[gi + j + 1]), make_float2(y.v[gi + j], y.v[gi + j + 1]),
+                             make_float2(z.v[gi + j], z.v[gi + j + 1]), make_float2((float)fx[j].gfx, (float)fx[j + 1].gfx),
+                             make_float2(fx[j].fr, fx[j + 1].fr), make_float2(s0.v[gi + j], s0.v[gi + j + 1]), A, cre, cim);
+              c[j] = make_float2(cre.x, cim.x);
+              c[j + 1] = make_float2(cre.y, cim.y);
+              ab[j] = __float_as_int(A.x);
+              ab[j + 1] = __float_as_int(A.y);
+            }
           }
         }
         // ---- gate, bin, weight and the guard-band test, from the two fixed-point coordinates ----
@@ -546,18 +560,30 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
         // ---- step A6: native int32 shared-memory reductions; whatever does not fit takes the cold block ----
         bool slow_any = false;
         bool slow[IL];
+        int r0[IL], r1[IL], r2[IL], r3[IL];   // round(value * weight * s) of the four reductions (1.5 * 2^23 trick), pairwise
+  #pragma unroll
+        for (int j = 0; j < IL; j += 2) {
+          const float2 fw = make_float2((float)(fx[j].gfx & (kFxOne - 1)), (float)(fx[j + 1].gfx & (kFxOne - 1)));
+          const float2 wAs = fma2(fw, bc(sS), bc(sO)), wBs = fma2(wAs, bc(-1.0f), bc(s));   // (w1, w0) s, or (w0, w1) s on swapped lanes
+          const float2 a0 = make_float2(sw_ri ? c[j].y : c[j].x, sw_ri ? c[j + 1].y : c[j + 1].x);
+          const float2 a1 = make_float2(sw_ri ? c[j].x : c[j].y, sw_ri ? c[j + 1].x : c[j + 1].y);
+          const float2 v0 = fma2(a0, wBs, bc(12582912.0f)), v1 = fma2(a1, wBs, bc(12582912.0f));
+          const float2 v2 = fma2(a0, wAs, bc(12582912.0f)), v3 = fma2(a1, wAs, bc(12582912.0f));
+          r0[j] = __float_as_int(v0.x) - 0x4B400000; r0[j + 1] = __float_as_int(v0.y) - 0x4B400000;
+          r1[j] = __float_as_int(v1.x) - 0x4B400000; r1[j + 1] = __float_as_int(v1.y) - 0x4B400000;
+          r2[j] = __float_as_int(v2.x) - 0x4B400000; r2[j + 1] = __float_as_int(v2.y) - 0x4B400000;
+          r3[j] = __float_as_int(v3.x) - 0x4B400000; r3[j + 1] = __float_as_int(v3.y) - 0x4B400000;
+        }
   #pragma unroll
         for (int j = 0; j < IL; ++j) {
           const int kw = k[j] - k0;
           const bool fits = ok[j] && !near[j] && (unsigned)kw < (unsigned)W && (unsigned)(ab[j] - lo_bits) <= fx_span;
-          const float wAs = fmaf((float)(fx[j].gfx & (kFxOne - 1)), sS, sO), wBs = s - wAs;             // (w1, w0) s, or (w0, w1) s on swapped lanes
-          const float a0 = sw_ri ? c[j].y : c[j].x, a1 = sw_ri ? c[j].x : c[j].y;
           const unsigned adr = tile_b + (unsigned)(g0[j] * RS4 + 4 * kw);
           if (fits) {
-            sh::red_add(adr, fx_round(a0, wBs));
-            sh::red_add(adr + d_ri, fx_round(a1, wBs));
-            sh::red_add(adr + d_lu, fx_round(a0, wAs));
-            sh::red_add(adr + d_lu + d_ri, fx_round(a1, wAs));
+            sh::red_add(adr, r0[j]);
+            sh::red_add(adr + d_ri, r1[j]);
+            sh::red_add(adr + d_lu, r2[j]);
+            sh::red_add(adr + d_lu + d_ri, r3[j]);
           }
           slow[j] = ok[j] && !fits;
           slow_any |= slow[j];

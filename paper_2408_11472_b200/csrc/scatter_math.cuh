@@ -158,8 +158,9 @@ __device__ __forceinline__ bool index_fast(const AccParams& p, const Pre& q, flo
 struct Fx {
   int gfx;     // floor(gf * 2^kFracBits)
   int kfx;     // floor((kf + 0.5) * 2^kFracBits); INT_MIN when |kf| >= 1024 (the fixed-point read would be meaningless)
-  float fr;    // frac(2R/lambda) mapped to [-0.5, 0.5) cycles
+  float fr;    // frac(2R/lambda) mapped to [-0.5, 0.5) cycles, in units of 2^-32 cycles
 };
+constexpr float kFrUnit = 2.3283064365386963e-10f;   // 2^-32: Fx::fr -> cycles
 
 template <int MODE>
 __device__ __forceinline__ Fx index_fx(const AccParams& p, const Pre& q, float xf, float yf, float zf, float vxf, float vyf,
@@ -181,7 +182,9 @@ __device__ __forceinline__ Fx index_fx(const AccParams& p, const Pre& q, float x
   }
   const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));
   o.kfx = (fabs(kf) < 1024.0) ? kfx : INT_MIN;
-  o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
+  // frac(2R/lambda) in units of 2^-32 cycles (two's complement wrap = the fraction in [-1/2, 1/2)): the magic number
+  // rides in the addend (fr0m = fr0 + 1.5 * 2^28, rounded to 2^-24 cycles)
+  o.fr = (float)(int)((unsigned)__double2loint(fma(gf, p.cq, p.fr0m)) << 8);
   return o;
 }
 
@@ -270,6 +273,49 @@ __device__ __forceinline__ float2 amplitude_t(const AccParams& p, float xf, floa
   A = sqrt_approx(s0dA) * ex2_approx(t * (inv_R2 * p.neg_alpha_log2e)) * inv_R2;
   return make_float2(A * cs, -A * sn);
 }
+// ---- packed fp32 pairs (sm_100: one instruction, two lanes of data): two scatterers at a time ----
+__device__ __forceinline__ unsigned long long pk(float2 a) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+  return r;
+}
+__device__ __forceinline__ float2 upk(unsigned long long r) {
+  float2 a;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+  return a;
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c)));
+  return upk(d);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+  unsigned long long d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+  return upk(d);
+}
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
+
+// Step A5 for TWO scatterers (components .x and .y of every argument), analytic gain: the same arithmetic as
+// amplitude_t<false>, with d.e1 and d.e2 taken straight from the coordinates (e1c = -r_sat.e1, e2c = -r_sat.e2 are host
+// constants) and the phase given in units of 2^-32 cycles (Fx::fr).  cre, cim: real and imaginary parts of the two amplitudes.
+__device__ __forceinline__ void amplitude_pair(const AccParams& p, float2 x, float2 y, float2 z, float2 gfx, float2 fr,
+                                               float2 s0dA, float2& A, float2& cre, float2& cim) {
+  const float2 inv_R2 = fma2(gfx, fma2(gfx, bc(p.a2), bc(p.a1)), bc(p.a0));
+  const float2 p1 = fma2(z, bc(p.e1z), fma2(y, bc(p.e1y), fma2(x, bc(p.e1x), bc(p.e1c))));
+  const float2 p2 = fma2(z, bc(p.e2z), fma2(y, bc(p.e2y), fma2(x, bc(p.e2x), bc(p.e2c))));
+  const float2 t = fma2(p2, p2, mul2(p1, p1));
+  const float2 arg = mul2(t, mul2(inv_R2, bc(p.neg_alpha_log2e)));
+  const float2 g = make_float2(sqrt_approx(s0dA.x) * ex2_approx(arg.x), sqrt_approx(s0dA.y) * ex2_approx(arg.y));
+  A = mul2(g, inv_R2);
+  const float2 ph = mul2(fr, bc(-6.283185307179586f * kFrUnit));   // -2 pi frac(2R/lambda)
+  float2 sn, cs;
+  __sincosf(ph.x, &sn.x, &cs.x);
+  __sincosf(ph.y, &sn.y, &cs.y);
+  cre = mul2(A, cs);
+  cim = mul2(A, sn);
+}
+
 // run-time choice (kernels off the hot path: reference, regular mode)
 __device__ __forceinline__ float2 amplitude(const AccParams& p, float xf, float yf, float zf, float gfx, float fr,
                                             float s0dA, float& A) {

@@ -155,6 +155,7 @@ void fast_path_constants(const sim_handle* h, const sim_sat_state* sat, AccParam
   {  // frac(rg0 * 2 / lambda) to ~1e-17 cycles: product split into rounded part + exact residual
     const double c = 2.0 / lam, q = rg0 * c, qe = std::fma(rg0, c, -q);
     p.fr0 = (q - std::floor(q)) + qe;
+    p.fr0m = p.fr0 + 402653184.0;   // 1.5 * 2^28
   }
   if (!(rg0 > 0)) return;
   const double margin = 0.01 * dR + 1e-9 * rg0;
@@ -297,6 +298,8 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
     const double e2[3] = {b[1] * e1[2] - b[2] * e1[1], b[2] * e1[0] - b[0] * e1[2], b[0] * e1[1] - b[1] * e1[0]};
     p.e1x = (float)e1[0]; p.e1y = (float)e1[1]; p.e1z = (float)e1[2];
     p.e2x = (float)e2[0]; p.e2y = (float)e2[1]; p.e2z = (float)e2[2];
+    p.e1c = (float)-((double)p.e1x * sat->pos[0] + (double)p.e1y * sat->pos[1] + (double)p.e1z * sat->pos[2]);
+    p.e2c = (float)-((double)p.e2x * sat->pos[0] + (double)p.e2y * sat->pos[1] + (double)p.e2z * sat->pos[2]);
     const double rg0 = sat->range_gate0_m, dRf = h->cfg.gate_spacing_m / (double)(1 << kFracBits);
     p.a0 = (float)(1.0 / (rg0 * rg0));
     p.a1 = (float)(-2.0 * dRf / (rg0 * rg0 * rg0));

@@ -32,6 +32,7 @@ struct AccParams {
   double pri, cP;         // pulse-pair Doppler: 1.0 / PRF and (-2.0 * N) / wavelength
   int doppler_mode;       // SIM_DOPPLER_*
   double fr0;             // frac(rg0 * 2 / lambda), exact to ~1e-17
+  double fr0m;            // fr0 + 1.5 * 2^28 (the magic number of the phase read rides in the addend)
   // ---- polynomial index path in u = R^2 - rg0^2: no sqrt, no divide ----
   int index_path;         // 0 canonical everywhere, 1 polynomial path + guard band
   int guard;              // guard band in units of 2^-kFracBits around integer gate boundaries
@@ -48,6 +49,7 @@ struct AccParams {
   float sxh, syh, szh, szl;            // satellite position as float (z as hi + lo)
   float neg_alpha_log2e;               // -antenna_alpha * log2(e)
   float e1x, e1y, e1z, e2x, e2y, e2z;  // orthonormal basis of the plane normal to the boresight
+  float e1c, e2c;                      // -r_sat.e1, -r_sat.e2 (with the fp32 basis vectors): d.e1 = r_p.e1 + e1c
   float a0, a1, a2;       // 1/R^2 = a0 + gfx (a1 + gfx a2), gfx = gf * 2^kFracBits
   float w_scale;          // 2^-kFracBits
   // ---- tabulated antenna gain on a u-v grid (reading R9); lut == nullptr: analytic gain ----
