@@ -232,10 +232,13 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   unsigned rd_nv = 0u;                 // valid count (0: none, the end of work has been reached)
   unsigned long long cp_base = 0ull;   // the chunk copied last
   unsigned cp_nv = 0u;
+  bool cp_first = false, rd_first = false;   // the chunk is the first of its scheduling unit
   auto copy_chunk = [&](unsigned st) {
     cp_nv = 0u;
+    cp_first = false;
     if (cs.left == 0u && !cs.stop) {   // (rare) the next unit
       stream_open(ut, cs);
+      cp_first = true;
       // the first warp to enter a unit (index cs.unit - 1) prepares a later one
       if (!cs.stop) {
         if (lane == 0 && sh::cas(claimed_a, (int)cs.unit - 1, (int)cs.unit) == (int)cs.unit - 1) {
@@ -270,6 +273,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   copy_chunk(0u);   // chunk 0 is in flight (two stages: the copies run one chunk ahead of the reads)
   rd_base = cp_base;
   rd_nv = cp_nv;
+  rd_first = cp_first;
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
@@ -359,6 +363,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     int ci = 0;
     for (; ci < EC; ++ci) {
       if (!DBG && dpend < e && sh::mbar_test(complete0 + 8u * (dpend & 1u), (dpend >> 1) & 1u)) try_drain(e, false);
+      // a scheduling unit that is not whole epochs (the ragged end of the input) ends its epoch early: the next unit lies
+      // elsewhere in the scene and gets its own Doppler window
+      if (ci > 0 && rd_first) break;
       // the next chunk goes into the stage that was read one iteration ago; then this lane's copies of the chunk to read
       // (one group older) must have landed
       copy_chunk(stg ^ 1u);
@@ -372,6 +379,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       const unsigned nvalid = rd_nv;
       rd_base = cp_base;
       rd_nv = cp_nv;
+      rd_first = cp_first;
 
       // ---- step A1: this lane's PT scatterers, shared-memory stage -> registers; the slice is refilled at once ----
       Vec<PT> x, y, z, vx, vy, vz, s0;
@@ -595,8 +603,14 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
               Idx t;
               if (MODE == kIdxCanonical) {
                 t = cx[j];
+              } else if (!near[j]) {
+                // outside the Doppler window or the fixed-point range of the epoch: the polynomial path's gate, bin,
+                // weight and amplitude stand, only the tile cannot take them
+                global_add(p, g0[j], k[j], (float)(fx[j].gfx & (kFxOne - 1)) * p.w_scale, c[j]);
+                ++escapes;
+                continue;
               } else {
-                if (near[j]) ++fallbacks;
+                ++fallbacks;
                 // the canonical sequence for every scatterer that leaves the tile (guard band or not: it is exact);
                 // offsets recomputed here (three subtractions) rather than kept alive across the amplitude for this rare case
                 const bool okj = canonical(p, __dsub_rn((double)x.v[gi + j], p.sx), __dsub_rn((double)y.v[gi + j], p.sy),
