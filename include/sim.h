@@ -107,7 +107,8 @@ int sim_workspace_bytes(const sim_config* cfg, size_t* out_bytes);
 
 /* Create a handle.  d_workspace: DEVICE pointer, 256-byte aligned, `bytes` >= sim_workspace_bytes,
  * owned by the caller and kept alive until sim_destroy.  cuda_stream: a cudaStream_t (NULL = the
- * legacy default stream).  Initialises the twiddle table on the stream. */
+ * legacy default stream).  Initialises the twiddle table on the stream.  Every call makes cfg.device current for its
+ * own duration and restores the caller's current device before it returns. */
 int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cuda_stream,
                sim_handle** out);
 

@@ -104,6 +104,18 @@ struct sim_handle {
 
 namespace {
 
+// Makes the handle's device current for the duration of a call and restores the caller's afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
 int fail(sim_handle* h, int code, const std::string& msg) {
   if (h) h->err = msg; else g_create_error = msg;
   return code;
@@ -501,8 +513,11 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   if (!d_workspace) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace is NULL");
   if (reinterpret_cast<uintptr_t>(d_workspace) & 255u) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace must be 256-byte aligned");
   if (bytes < lay.total) return fail(nullptr, SIM_ERR_WORKSPACE, "workspace smaller than sim_workspace_bytes");
-  cudaError_t e = cudaSetDevice(cfg->device);
-  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaSetDevice");
+  int n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount");
+  if (cfg->device >= n_dev) return fail(nullptr, SIM_ERR_BAD_CONFIG, "cfg.device is not a CUDA device of this process");
+  DeviceGuard guard(cfg->device);   // the caller's current device is restored on return
   sim_handle* h = new (std::nothrow) sim_handle();
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "out of host memory");
   h->cfg = *cfg;
@@ -568,6 +583,7 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
 }
 
 int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   float2* T = nullptr;
   int rc = begin_update(h, d_scat, sat, flags, true, &T);
   if (rc) return rc;
@@ -590,6 +606,7 @@ int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim
 }
 
 int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, const sim_sat_state* sat, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (h && h->cfg.host_stage_scatterers <= 0) return fail(h, SIM_ERR_INVALID_ARG, "host staging disabled (cfg.host_stage_scatterers == 0)");
   float2* T = nullptr;
   int rc = begin_update(h, h_scat, sat, flags, false, &T);
@@ -652,6 +669,7 @@ int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, cons
 }
 
 int sim_synthesize_pulses(sim_handle* h, int64_t n_pulses, void* d_iq, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   int64_t s0 = 0, s1 = -1;
   int rc = plan_synthesis(h, n_pulses, d_iq, flags, &s0, &s1);
   if (rc || n_pulses == 0) return rc;
@@ -660,6 +678,7 @@ int sim_synthesize_pulses(sim_handle* h, int64_t n_pulses, void* d_iq, uint32_t 
 }
 
 int sim_synthesize_pulses_host(sim_handle* h, int64_t n_pulses, void* h_iq, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (h && n_pulses > h->cfg.host_stage_pulses) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses exceeds cfg.host_stage_pulses");
   int64_t s0 = 0, s1 = -1;
   int rc = plan_synthesis(h, n_pulses, h_iq, flags, &s0, &s1);
@@ -674,6 +693,7 @@ int sim_synthesize_pulses_host(sim_handle* h, int64_t n_pulses, void* h_iq, uint
 
 int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, int64_t first_pulse,
                        int64_t n_pulses, void* d_iq, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (flags & ~SIM_ACC_APPEND) return fail(h, SIM_ERR_INVALID_ARG, "unknown regular-mode flag");
   if (n_pulses < 0 || n_pulses > (1 << 24)) return fail(h, SIM_ERR_INVALID_ARG, "n_pulses outside 0..2^24");
@@ -703,6 +723,7 @@ int sim_regular_pulses(sim_handle* h, const sim_scatterers* d_scat, const sim_sa
 }
 
 int sim_burst_beams(sim_handle* h, const void* d_iq, int64_t n_pulses, int32_t burst, void* d_beams, uint32_t flags) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (flags) return fail(h, SIM_ERR_INVALID_ARG, "unknown burst flag");
   if (burst < 16 || burst > 128 || (burst & (burst - 1))) return fail(h, SIM_ERR_INVALID_ARG, "burst must be a power of two in 16..128");
@@ -722,6 +743,7 @@ int sim_burst_beams(sim_handle* h, const void* d_iq, int64_t n_pulses, int32_t b
 }
 
 int sim_synchronize(sim_handle* h) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   cudaError_t e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamSynchronize");
@@ -747,6 +769,7 @@ int sim_destroy(sim_handle* h) {
 }
 
 int sim_get_spectrum(sim_handle* h, int64_t update_index, void* d_out) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (!d_out) return fail(h, SIM_ERR_INVALID_ARG, "d_out is NULL");
   if (update_index < 0 || update_index >= h->n_updates || update_index < h->n_updates - h->cfg.max_pending_updates)
@@ -767,6 +790,7 @@ int sim_spectrum_offset(sim_handle* h, int64_t update_index, size_t* out_offset)
 }
 
 int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, int32_t* d_gate0, int32_t* d_bin) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (!d_scat) return fail(h, SIM_ERR_INVALID_ARG, "scatterers is NULL");
   if (d_scat->n && (!d_gate0 || !d_bin)) return fail(h, SIM_ERR_INVALID_ARG, "output arrays are NULL");
@@ -806,6 +830,7 @@ int sim_set_antenna_lut(sim_handle* h, const void* d_table, int32_t n_u, int32_t
 }
 
 int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (value < 0) return fail(h, SIM_ERR_INVALID_ARG, "option value < 0");
   // options that change the launch shape are re-planned; a shape the kernels do not support restores the old value
@@ -901,6 +926,7 @@ int sim_get_stats(const sim_handle* h, sim_stats* out) {
 }
 
 int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset) {
+  DeviceGuard guard(h ? h->cfg.device : 0);
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (!h_out) return fail(h, SIM_ERR_INVALID_ARG, "h_out is NULL");
   cudaError_t e = cudaMemcpyAsync(h_out, counters(h), 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, h->stream);

@@ -621,3 +621,21 @@ def test_argument_errors(sim_mod):
     assert sim.stats()["updates_accumulated"] == 0   # errors leave the handle unchanged
     sim.accumulate_update(scat, sim_mod.sat_for(wl, 0))
     assert sim.stats()["updates_accumulated"] == 1 and sim.stats()["kernel_launches"] >= 2
+
+
+def test_two_live_handles_with_different_shapes(oracle, sim_mod):
+    """Distinct handles are independent (include/sim.h): the dynamic shared-memory limit of a kernel is per function and
+    per device, so a handle planned for a smaller tile must not break the launches of one that needs more."""
+    wl_a = W.get("tiny").scaled(n_gates=128, n_doppler=256, pulses_per_update=256, n_updates=1)
+    wl_b = W.get("tiny").scaled(n_gates=64, n_doppler=64, pulses_per_update=64, n_updates=1)
+    scat = W.scatterers(wl_a)
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    sims = {}
+    for name, wl in (("a", wl_a), ("b", wl_b)):        # create a (large tile) first, then b (small tile)
+        sims[name] = (wl, sim_mod.Sim(sim_mod.config_for(wl, max_pending_updates=4)), U.oracle_spectra(oracle, wl, scat_np, [0])[0])
+    for rnd in range(3):                                # accumulate alternately
+        for name in ("a", "b"):
+            wl, sim, T_ref = sims[name]
+            sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+            assert U.rel_l2(sim.get_spectrum(rnd).cpu().numpy(), T_ref) <= U.TOL, (name, rnd)
+            sim.synthesize_pulses(wl.pulses_per_update, flags=sim_mod.SYN_FINAL)
