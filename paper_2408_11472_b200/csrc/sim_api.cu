@@ -484,7 +484,7 @@ int do_synthesize(sim_handle* h, int64_t n_pulses, float2* d_iq, int64_t s_first
   p.N = h->cfg.n_doppler;
   p.P = h->cfg.pulses_per_update;
   p.n_segments = s_last - s_first + 1;
-  synth_plan(p.N, p.G, p.n_segments, h->sm_count, &p.GT, &p.seg_per_block);
+  synth_plan(p.N, p.G, p.P, p.n_segments, h->sm_count, &p.GT, &p.seg_per_block);
   p.weight_mode = h->cfg.weight_mode;
   int l = 0;
   cudaError_t e = launch_synthesize(p, h->stream, &l);
@@ -569,7 +569,7 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->smem_per_sm = (size_t)v;
   e = plan_ws(h);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "accumulation kernel occupancy query"); }
-  e = synth_prepare(cfg->n_doppler);
+  e = synth_prepare(cfg->n_doppler, cfg->pulses_per_update);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "synthesis kernel shared-memory attribute"); }
   e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(unsigned int), h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->ws + lay.t64_off, 0, lay.t64_bytes, h->stream);

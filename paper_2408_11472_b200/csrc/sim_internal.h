@@ -85,6 +85,7 @@ struct SynParams {
   int GT;                 // gates per block
   int seg_per_block;      // consecutive segments per block (each spectrum is transformed once per run)
   int n_pass, radix[kSynMaxPass];   // Stockham passes: N = product of the radices (4, 2, 3, 5)
+  int pass_m[kSynMaxPass], pass_ns[kSynMaxPass], pass_tstep[kSynMaxPass];   // butterflies per signal, product of the earlier radices, twiddle step
   int weight_mode;
 };
 
@@ -115,8 +116,8 @@ cudaError_t launch_burst_fft(const float2* Y, float2* Z, long long n_bursts, int
                              int* launches);
 cudaError_t launch_twiddles(float2* tw, int N, cudaStream_t st, int* launches);
 cudaError_t launch_synthesize(const SynParams& p, cudaStream_t st, int* launches);
-void synth_plan(int N, int G, long long n_segments, int sm_count, int* gt, int* seg_per_block);
+void synth_plan(int N, int G, int P, long long n_segments, int sm_count, int* gt, int* seg_per_block);
 bool synth_factor(int N, int* radix, int* n_pass);
-cudaError_t synth_prepare(int N);
+cudaError_t synth_prepare(int N, int P);
 
 }  // namespace simk

@@ -40,14 +40,16 @@ bool synth_factor(int N, int* radix, int* n_pass) {
   return n == 1 && k <= kSynMaxPass;
 }
 
-size_t synth_smem_bytes(int N, int GT) { return ((size_t)3 * GT * (N + 1) + N) * sizeof(float2); }
+constexpr int kSynMaxWeightTable = 4096;   // pulses per update up to which eq. (1) is tabulated once per block
+static int synth_weight_entries(int P) { return P <= kSynMaxWeightTable ? P : 0; }
+size_t synth_smem_bytes(int N, int GT, int P) { return ((size_t)3 * GT * (N + 1) + N + synth_weight_entries(P)) * sizeof(float2); }
 
 // Gates per block and segments per block.  Three signal buffers of GT rows must fit; a long call (many segments)
 // uses 8-gate tiles (64-byte IQ pieces) and runs of segments that still give about two blocks per SM; a short call
 // takes smaller tiles so that it has blocks at all.
-void synth_plan(int N, int G, long long n_segments, int sm_count, int* gt_out, int* seg_per_block) {
+void synth_plan(int N, int G, int P, long long n_segments, int sm_count, int* gt_out, int* seg_per_block) {
   int gt = 8;
-  while (gt > 1 && synth_smem_bytes(N, gt) > 100 * 1024) gt >>= 1;
+  while (gt > 1 && synth_smem_bytes(N, gt, P) > 100 * 1024) gt >>= 1;
   while (gt > 2 && n_segments * ((G + gt - 1) / gt) < sm_count / 2) gt >>= 1;
   const long long tiles = (G + gt - 1) / gt;
   long long runs = (2LL * sm_count + tiles - 1) / tiles;   // runs of segments wanted per gate tile
@@ -112,8 +114,8 @@ __device__ __forceinline__ void idft_small<5>(float2* v) {
 // dst[(j - j mod Ns) R + (j mod Ns) + t Ns].  POW2: N/R and Ns are powers of two (every index is a shift or a mask).
 template <int R, bool POW2>
 __device__ __forceinline__ void stockham_pass(const float2* __restrict__ src, float2* __restrict__ dst, const float2* __restrict__ tw,
-                                              int rows, int N, int LD, int Ns, int tid) {
-  const int M = N / R, tstep = M / Ns;   // twiddle index k t N / (Ns R) < N: no reduction needed
+                                              int rows, int M, int LD, int Ns, int tstep, int tid) {
+  // M = N / R butterflies per signal; tstep = M / Ns: twiddle index k t N / (Ns R) < N needs no reduction
   const int logM = 31 - __clz(M);
   for (int e = tid; e < rows * M; e += kSynThreads) {
     const int row = POW2 ? (e >> logM) : (e / M), j = POW2 ? (e & (M - 1)) : (e - row * M);
@@ -146,34 +148,59 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
   const long long s_end = min(s_begin + p.seg_per_block, p.seg0 + p.n_segments);
 
   for (int j = tid; j < N; j += kSynThreads) tw[j] = p.tw[j];
+  // eq. (1) for every pulse offset of a segment, once per block: wt[m] = (W_s, W_{s+1}) at a = m / P
+  const int P = p.P;
+  const float invP = 1.0f / (float)P;
+  float2* wt = buf0 + 3 * bufsz;
+  const bool tabulated = P <= kSynMaxWeightTable;
+  auto weights = [&](int m) {
+    const float a = (float)m * invP;
+    float ws = 1.0f - a, wn = a;
+    if (p.weight_mode == SIM_W_SQRT) {
+      ws = sqrtf(ws);
+      wn = sqrtf(wn);
+    }
+    return make_float2(ws, wn);
+  };
+  if (tabulated)
+    for (int m = tid; m < P; m += kSynThreads) wt[m] = weights(m);
 
   const bool pow2 = (N & (N - 1)) == 0;
-  const int logN = 31 - __clz(N), logGT = 31 - __clz(GT);
+  const int logGT = 31 - __clz(GT), logN = 31 - __clz(N);
   // S1 of spectrum u: rows of T_u -> buffer `a` (straight copy), passes between `a` and `b`; returns where y_u ended up
   auto transform = [&](long long u, float2* a, float2* b) -> float2* {
     const float2* T = p.ring + (size_t)(u % p.cap) * p.slot_stride + (size_t)gbase * N;
-    if (pow2) {
-#pragma unroll 4
-      for (int e = tid; e < rows * N; e += kSynThreads) a[(size_t)(e >> logN) * LD + (e & (N - 1))] = T[e];
-    } else {
-      for (int row = 0; row < rows; ++row)
-        for (int j = tid; j < N; j += kSynThreads) a[(size_t)row * LD + j] = T[(size_t)row * N + j];
+    // batches of eight loads per thread in flight before the first store (the rows of a tile are contiguous in T)
+    const int total = rows * N;
+    for (int base = tid; base < total; base += 8 * kSynThreads) {
+      float2 r[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int e = base + i * kSynThreads;
+        if (e < total) r[i] = __ldg(T + e);
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int e = base + i * kSynThreads;
+        if (e < total) {
+          const int rw = pow2 ? (e >> logN) : (e / N);
+          a[(size_t)rw * LD + (e - rw * N)] = r[i];
+        }
+      }
     }
     __syncthreads();
-    int Ns = 1;
     for (int ps = 0; ps < p.n_pass; ++ps) {
-      const int R = p.radix[ps];
+      const int R = p.radix[ps], M = p.pass_m[ps], Ns = p.pass_ns[ps], ts = p.pass_tstep[ps];
       if (pow2) {
-        if (R == 4) stockham_pass<4, true>(a, b, tw, rows, N, LD, Ns, tid);
-        else stockham_pass<2, true>(a, b, tw, rows, N, LD, Ns, tid);
+        if (R == 4) stockham_pass<4, true>(a, b, tw, rows, M, LD, Ns, ts, tid);
+        else stockham_pass<2, true>(a, b, tw, rows, M, LD, Ns, ts, tid);
       } else {
-        if (R == 4) stockham_pass<4, false>(a, b, tw, rows, N, LD, Ns, tid);
-        else if (R == 2) stockham_pass<2, false>(a, b, tw, rows, N, LD, Ns, tid);
-        else if (R == 3) stockham_pass<3, false>(a, b, tw, rows, N, LD, Ns, tid);
-        else stockham_pass<5, false>(a, b, tw, rows, N, LD, Ns, tid);
+        if (R == 4) stockham_pass<4, false>(a, b, tw, rows, M, LD, Ns, ts, tid);
+        else if (R == 2) stockham_pass<2, false>(a, b, tw, rows, M, LD, Ns, ts, tid);
+        else if (R == 3) stockham_pass<3, false>(a, b, tw, rows, M, LD, Ns, ts, tid);
+        else stockham_pass<5, false>(a, b, tw, rows, M, LD, Ns, ts, tid);
       }
       __syncthreads();
-      Ns *= R;
       float2* t = a; a = b; b = t;
     }
     return a;
@@ -186,8 +213,13 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
     float2* r = transform(s_begin, cur, f1);
     if (r != cur) { f1 = cur; cur = r; }
   }
-  const float invP = 1.0f / (float)p.P;
-  const int P = p.P;
+  // one thread = one gate row of the tile and every (256 / GT)-th pulse of the segment: row, base pointers and the
+  // output stride are loop invariants, the sample indices advance by additions
+  const int row = tid & (GT - 1), pi0 = tid >> logGT, pstep = kSynThreads >> logGT;
+  const size_t ostep = (size_t)pstep * p.G;
+  int off_n = (-P) % N;            // (m - P) mod N = (m + off_n) mod N, off_n in [0, N)
+  off_n += off_n < 0 ? N : 0;
+  const int pstep_n = pstep % N;
   for (long long s = s_begin; s < s_end; ++s) {
     const bool has_next = (s + 1 < p.n_spectra);
     float2* nxt = nullptr;
@@ -199,32 +231,26 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
     const long long seg_lo = s * (long long)P;
     const long long lo = max(seg_lo, p.x0), hi = min(seg_lo + P, p.x0 + p.n_pulses);
     const int npul = (int)(hi - lo);
-    int off_n = (-P) % N;            // (m - P) mod N = (m + off_n) mod N, off_n in [0, N)
-    off_n += off_n < 0 ? N : 0;
-    for (int e = tid; e < (npul << logGT); e += kSynThreads) {
-      const int pi = e >> logGT, row = e & (GT - 1);
-      if (row >= rows) continue;
-      const long long x = lo + pi;
-      const int m = (int)(x - seg_lo);  // 0..P-1
-      int ms = m;
-      while (ms >= N) ms -= N;          // P / N turns at most
-      const float2 ys = cur[(size_t)row * LD + ms];
-      float2 out;
-      if (has_next) {
-        const float a = (float)m * invP;
-        float ws = 1.0f - a, wn = a;
-        if (p.weight_mode == SIM_W_SQRT) {
-          ws = sqrtf(ws);
-          wn = sqrtf(wn);
+    if (row < rows) {
+      const float2* crow = cur + (size_t)row * LD;
+      const float2* nrow = has_next ? nxt + (size_t)row * LD : crow;
+      float2* outp = p.iq + (size_t)(lo - p.x0 + pi0) * p.G + gbase + row;
+      int m = (int)(lo - seg_lo) + pi0;   // 0..P-1
+      int ms = m % N;
+      for (int pi = pi0; pi < npul; pi += pstep, m += pstep, outp += ostep) {
+        const float2 ys = crow[ms];
+        float2 out = ys;   // tail rule: a lone spectrum at weight 1
+        if (has_next) {
+          int mn = ms + off_n;
+          mn -= mn >= N ? N : 0;
+          const float2 yn = nrow[mn];
+          const float2 w = tabulated ? wt[m] : weights(m);
+          out = make_float2(w.x * ys.x + w.y * yn.x, w.x * ys.y + w.y * yn.y);
         }
-        int mn = ms + off_n;
-        mn -= mn >= N ? N : 0;
-        const float2 yn = nxt[(size_t)row * LD + mn];
-        out = make_float2(ws * ys.x + wn * yn.x, ws * ys.y + wn * yn.y);
-      } else {
-        out = ys;  // tail rule: lone spectrum at weight 1
+        *outp = out;
+        ms += pstep_n;
+        ms -= ms >= N ? N : 0;
       }
-      p.iq[(size_t)(x - p.x0) * p.G + gbase + row] = out;
     }
     __syncthreads();   // the emission has read `cur`: it becomes a free buffer
     if (has_next) {
@@ -234,17 +260,22 @@ __global__ void __launch_bounds__(kSynThreads) synth_kernel(SynParams p) {
 }
 
 // Once per handle: the dynamic shared-memory limit of the kernel (largest plan for this N).
-cudaError_t synth_prepare(int N) {
+cudaError_t synth_prepare(int N, int P) {
   int gt = 8;
-  while (gt > 1 && synth_smem_bytes(N, gt) > 100 * 1024) gt >>= 1;
-  return cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synth_smem_bytes(N, gt));
+  while (gt > 1 && synth_smem_bytes(N, gt, P) > 100 * 1024) gt >>= 1;
+  return cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synth_smem_bytes(N, gt, P));
 }
 
 cudaError_t launch_synthesize(const SynParams& p0, cudaStream_t st, int* launches) {
   if (p0.n_segments <= 0 || p0.n_pulses <= 0) return cudaSuccess;
   SynParams p = p0;
   if (!synth_factor(p.N, p.radix, &p.n_pass)) return cudaErrorInvalidValue;
-  const size_t smem = synth_smem_bytes(p.N, p.GT);
+  for (int ps = 0, ns = 1; ps < p.n_pass; ns *= p.radix[ps], ++ps) {   // per-pass constants of the Stockham scheme
+    p.pass_m[ps] = p.N / p.radix[ps];
+    p.pass_ns[ps] = ns;
+    p.pass_tstep[ps] = p.pass_m[ps] / ns;
+  }
+  const size_t smem = synth_smem_bytes(p.N, p.GT, p.P);
   // per launch: the limit is per function and per device, another handle may have set it for a smaller N
   cudaError_t e = cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
