@@ -167,7 +167,7 @@ def test_p2_pure_tone(oracle, k):
 
 
 # ---- P3 / P4: library special case and Parseval (invariant (d)) ----------------------------------
-@pytest.mark.parametrize("N", [16, 64, 512, 12, 1])
+@pytest.mark.parametrize("N", [16, 64, 512, 12, 1, 250, 750, 1250])   # (the paper's n_fast values: any N)
 def test_p3_idft_is_N_times_numpy_ifft(oracle, N):
     rng = np.random.default_rng(N)
     T = rng.normal(size=(5, N)) + 1j * rng.normal(size=(5, N))
@@ -260,7 +260,7 @@ def test_synthesize_tail_and_not_ready(oracle):
     assert np.array_equal(Yp, Y[5:25])
 
 
-@pytest.mark.parametrize("N,P", [(16, 16), (32, 16), (16, 12), (64, 100)])
+@pytest.mark.parametrize("N,P", [(16, 16), (32, 16), (16, 12), (64, 100), (250, 250), (500, 250)])
 def test_o3_definition_against_numpy(oracle, N, P):
     """O3 written a second time with numpy.fft and explicit eq. (1) weights (periodic extension, A4)."""
     rng = np.random.default_rng(N + P)
