@@ -201,29 +201,23 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
                       int32_t* d_gate0, int32_t* d_bin);
 
 /* Tuning knobs (benchmarks and tests; defaults are chosen by the library). */
-#define SIM_OPT_ACC_VARIANT 1   /* 0 = reference kernel (global atomics), 1 = barrier-synchronised tile kernel,
-                                   2 = warp-specialised tile kernel (control warp + compute warps),
-                                   3 = producer warp + drain warp + compute warps, long epochs (default).
-                                   Selecting a variant resets warps / per-lane / epoch options to its defaults */
-#define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto */
-#define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit; 0 = auto */
-#define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto (variant 3: any width, 12 or 16 by
-                                     default; variants 1, 2: a power of two) */
+#define SIM_OPT_ACC_VARIANT 1   /* 4 = production kernel (default), 0 = reference kernel (one thread per scatterer, canonical
+                                   sequence, global fp64 reductions; the A/B partner in the parity tests).
+                                   Selecting a variant resets warps / per-lane / epoch options to the defaults */
+#define SIM_OPT_ACC_BLOCKS 2    /* grid size of the accumulation kernel; 0 = auto (resident blocks x SMs) */
+#define SIM_OPT_ACC_SUPERCHUNK 3 /* scatterers per scheduling unit (rounded up to whole fixed-point epochs); 0 = auto */
+#define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto (as many as fit, up to 20) */
 #define SIM_OPT_GUARD_LSB 5     /* guard band of the fast index path in units of 2^-20 gate / bin (default 16) */
-#define SIM_OPT_ACC_PER_THREAD 7 /* scatterers per thread per chunk of the tile kernel: 2 or 4 */
-#define SIM_OPT_ACC_MIN_BLOCKS 8 /* register budget of the tile kernel: compiled for 2..4 resident blocks per SM */
-#define SIM_OPT_ACC_WARPS 9      /* compute warps per block.  variant 2: 7, 14 (default), 22 or 30;
-                                    variant 3 (with per-lane, interleave): (8,4,4) default, (8,2,2), (8,4,2),
-                                    (12,2,2), (16,4,2), (20,4,2) */
-#define SIM_OPT_ACC_STAGES 10    /* depth of the TMA stage ring: 0 = as many as fit, else 2..4 (variant 3: 2..6) */
-#define SIM_OPT_ACC_PER_LANE 11  /* variant 3: scatterers per lane per chunk: 2 or 4 */
-#define SIM_OPT_ACC_EPOCH 12     /* scatterers per fixed-point epoch: variant 2 64..2047 (default 2047), variant 3 64..16383 (default 8191) */
-#define SIM_OPT_ACC_WAIT_HINT 13 /* variant 3: suspend-time hint (ns) of the compute warps' mbarrier waits; 0 (default) =
-                                    plain try_wait loop (the control warps always sleep) */
-#define SIM_OPT_ACC_SCATTER 14   /* variant 3: 1 (default) = scheduling units visit the scene in a scattered order (dark and
-                                    illuminated parts in flight together), 0 = in order */
-#define SIM_OPT_ACC_INTERLEAVE 15 /* variant 3: scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
-#define SIM_OPT_ACC_SHAPE 16      /* block shape in one call: (warps << 16) | (per lane << 8) | interleave */
+#define SIM_OPT_ACC_WARPS 9      /* warps per block: 8 (default, two blocks per SM) or 16 */
+#define SIM_OPT_ACC_STAGES 10    /* accepted and ignored (the production kernel copies one chunk ahead: two stages) */
+#define SIM_OPT_ACC_PER_LANE 11  /* scatterers per lane per chunk: 2 or 4 (default) */
+#define SIM_OPT_ACC_EPOCH 12     /* scatterers per fixed-point epoch: 64..16383 (default 8191) */
+#define SIM_OPT_ACC_WAIT_HINT 13 /* accepted and ignored */
+#define SIM_OPT_ACC_SCATTER 14   /* 1 (default) = scheduling units visit the scene in a scattered order (dark and
+                                    illuminated parts in flight together); 0 = in input order */
+#define SIM_OPT_ACC_INTERLEAVE 15 /* scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
+#define SIM_OPT_ACC_SHAPE 16      /* block shape in one call: (warps << 16) | (per lane << 8) | interleave;
+                                     compiled shapes: (8,4,4) default, (8,4,2), (8,2,2), (16,4,4) */
 #define SIM_OPT_INDEX_PATH 6    /* 0 = canonical fp64 sequence everywhere, 1 = fast path + guard band (default) */
 int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 

@@ -11,7 +11,7 @@ CSRC = os.path.join(_HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(CSRC, "libsim.so")
-SOURCES = ["sim_api.cu", "accumulate.cu", "accumulate_ws3.cu", "synthesize.cu", "regular.cu", "burst.cu"]
+SOURCES = ["sim_api.cu", "accumulate.cu", "synthesize.cu", "regular.cu", "burst.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "shared"]
 

@@ -2,34 +2,34 @@
 // sm_100a, no tensor cores: a streaming scan of 28 B per scatterer with a scatter-add, bounded by HBM bandwidth,
 // instruction issue and the shared-memory atomic unit.
 //
-// Production kernel `acc_kernel` (variant 4).  Persistent blocks, two per SM, NCW = 8 warps that all compute (128
-// registers per thread; a block of 9 or 10 warps gets 96):
-//   * scheduling units of consecutive scatterers are drawn from a global ticket counter (visited in a scattered order so
-//     that dark and illuminated parts of the scene are in flight together) and streamed in chunks of CH = NCW*32*PT
-//     through a ring of shared-memory stages by per-lane 16-byte asynchronous copies (cp.async.cg, LDGSTS: a warp
-//     instruction moves 512 contiguous bytes of one array).  There is no producer warp, no mbarrier and no hand-shake
-//     between warps on the load side: every lane copies exactly the 7 x 16 bytes it will read itself, one chunk ahead
-//     per extra stage, and waits for its own commit groups.  (Round 1 and the first versions of this kernel used TMA bulk
-//     copies issued by one lane per block or per warp: the uniform-register set-up of seven bulk copies per 4 KB slice
-//     cost more issue slots than it saved, and a refill that waits for the slowest warp of the block starved the fast
-//     ones.)  The sequence of chunks (base, count) is a small table in shared memory that whichever warp gets there
-//     first extends under a lock;
-//   * steps A2-A5 run in registers for IL scatterers at a time: range and phase in fp64 (polynomial in u = R^2 - rg0^2),
-//     Doppler coordinate in fp32 with a proven error bound, amplitude in fp32; gate, bin and the guard-band test are
-//     derived last, from two fixed-point integers, and the rare cases (guard band, outside the Doppler window, outside
-//     the fixed-point range) go through ONE cold block per group where the canonical fp64 sequence decides;
+// Production kernel `acc_kernel` (variant 4).  Persistent blocks, two per SM, NCW = 8 warps that all compute (up to 128
+// registers per thread):
+//   * scheduling units of consecutive scatterers (whole fixed-point epochs) are drawn from a global ticket counter
+//     (visited in a scattered order so that dark and illuminated parts of the scene are in flight together) and streamed
+//     in chunks of CH = NCW*32*PT through a two-stage shared-memory ring by per-lane 16-byte asynchronous copies
+//     (cp.async.cg, LDGSTS: a warp instruction moves 512 contiguous bytes of one array).  There is no producer warp and no
+//     hand-shake between warps on the load side: every lane copies exactly the 7 x 16 bytes it will read itself, one chunk
+//     ahead, and waits for its own commit group.  (Round 1 used TMA bulk copies issued by a producer warp; per-warp bulk
+//     copies and plain ld.global.nc prefetch into registers were measured this round and lost: DESIGN.md section 6.)
+//     The units (start, end) sit in a small shared-memory table that the first warp into unit u extends by unit u + 2;
+//     a partial unit (ragged end of the input) ends its epoch early;
+//   * steps A2-A5 run in registers for IL scatterers at a time: range, gate and Doppler coordinates and the phase in fp64
+//     (polynomials in u = R^2 - rg0^2), amplitude in packed fp32 (fma/mul.rn.f32x2: two scatterers per instruction); gate,
+//     bin and the guard-band test are derived last, from two fixed-point integers; the rare cases go through ONE cold
+//     block per group: guard-band cases are decided by the canonical fp64 sequence, window and range escapes keep their
+//     indices and go to the global accumulator;
 //   * step A6 is block floating point: native int32 shared-memory reductions (red.shared.add.s32) of round(w c s) into a
-//     tile of FOUR planes [lower-gate half | upper-gate half] x [re | im], each [G+1][W]; s is a power of two fixed per
+//     tile of FOUR planes [lower-gate half | upper-gate half] x [re | im], each [G+1][RS]; s is a power of two fixed per
 //     epoch of <= 8191 scatterers from the geometric mean of the first warp's amplitudes, so that no cell can overflow.
-//     3 000-20 000 scatterers land in each hot cell and a warp's 32 scatterers hit only ~8 distinct cells, so same-address
-//     replays dominate the atomic unit; the four values of a scatterer are therefore issued in a lane-dependent order
-//     (lane bit 0 swaps re/im, lane bit 1 swaps lower/upper): every reduction instruction spreads its 32 lanes over all
-//     four planes and the replays per instruction drop from ~9.8 to ~6.5 (profiles/);
-//   * when the last warp has finished an epoch, every warp drains ITS SHARE of that epoch's gate rows into fp64 global
-//     reductions (step A7) at its next chunk boundary, while the second tile already fills with the next epoch: no drain
-//     warp, no rendez-vous, nobody falls behind by more than an eighth of a drain.  The global accumulator is an
-//     fp64 grid (exact enough that 10^5 identical escapes into one cell lose nothing); `acc_finalize_kernel` rounds it
-//     to the complex64 spectrum and re-zeroes it.
+//     3 000-20 000 scatterers land in each hot cell and a warp's 32 scatterers hit only ~9 distinct cells, so same-address
+//     and same-bank replays are what the atomic unit spends its time on; the four values of a scatterer are therefore
+//     issued in a lane-dependent order (lane bit 0 swaps re/im, lane bit 1 swaps lower/upper) and rows and planes are
+//     padded (acc_row_stride, acc_plane_words below): 4.1 wavefronts per reduction instruction instead of 9.4;
+//   * when the last warp has finished an epoch (an mbarrier phase per tile), every warp drains ITS SHARE of that epoch's
+//     gate rows into fp64 global reductions (step A7) at its next chunk boundary, while the second tile already fills
+//     with the next epoch: no drain warp, no rendez-vous; a warp that runs ahead sleeps on the mbarrier.  The global
+//     accumulator is an fp64 grid (exact enough that 10^5 identical escapes into one cell lose nothing);
+//     `acc_finalize_kernel` rounds it to the complex64 spectrum and re-zeroes it.
 // Reference kernel `acc_reference_kernel` (variant 0): one thread per scatterer, canonical sequence, global fp64
 // reductions; the A/B partner of the production kernel in the parity tests.
 // `sim_debug_indices` runs the production kernel itself with DBG = true (same index flow, indices written instead of

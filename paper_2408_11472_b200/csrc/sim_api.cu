@@ -86,7 +86,7 @@ struct sim_handle {
   // tuning
   int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard;
   int64_t opt_superchunk;
-  int opt_ncw, opt_stages;          // compute warps per block, TMA ring depth (0 = auto)
+  int opt_ncw, opt_stages;          // warps per block; ring depth option (accepted, unused)
   int ws_W, ws_stages, ws_blocks_per_sm;   // planned window width, ring depth, resident blocks per SM
   int opt_wait_hint, opt_scatter;
   int opt_il;
@@ -231,39 +231,22 @@ cudaError_t plan_ws(sim_handle* h) {
     return cudaSuccess;
   }
   const int G = h->cfg.n_gates, N = h->cfg.n_doppler, ncw = h->opt_ncw, pt = h->opt_pt;
-  const bool v3 = h->opt_variant == 3;
-  if (v3 ? !acc_ws3_supported(ncw, pt, h->opt_il) : !acc_supported(ncw, pt, h->opt_il)) return cudaErrorInvalidValue;
-  auto smem = [&](int g, int w, int st) { return v3 ? acc_ws3_smem_bytes(g, w, ncw, pt, st) : acc_smem_bytes(g, w, ncw, pt, st); };
+  if (!acc_supported(ncw, pt, h->opt_il)) return cudaErrorInvalidValue;
+  auto smem = [&](int g, int w, int st) { return acc_smem_bytes(g, w, ncw, pt, st); };
   const int target = ncw <= 8 ? 2 : 1;                              // blocks per SM the register budget allows
   size_t budget = h->smem_per_sm / target;
   budget = budget > 2048 ? budget - 2048 : 0;                       // 1 KB reserved per block + static shared memory
   if (budget > h->smem_optin - 4096) budget = h->smem_optin - 4096;   // the kernels' static shared memory (< 3 KB) counts against the opt-in limit
   const size_t stage = smem(0, 0, 1) - smem(0, 0, 0);
-  int w = h->opt_window > 0 ? h->opt_window : (v3 ? 16 : 20);
+  const int st = 2;   // every lane copies one chunk ahead of its reads: two stages
+  int w = h->opt_window > 0 ? h->opt_window : 20;
   if (w > N) w = N;
-  auto tiles_of = [&](int ww) { return smem(G, ww, 0); };
-  while (w > 1 && tiles_of(w) + 2 * stage > budget) --w;
-  int st = tiles_of(w) + 2 * stage <= budget ? (int)((budget - tiles_of(w)) / stage) : 2;
-  if (v3 && h->opt_window == 0 && st < 3) {
-    // a third stage is worth more than the last bins of the window (measured on the 268M config; below 12 bins the
-    // escapes take over)
-    for (int w2 = w - 1; w2 >= 12 && w2 >= 3 * w / 4; --w2) {
-      if (tiles_of(w2) + 3 * stage <= budget) {
-        w = w2;
-        st = 3;
-        break;
-      }
-    }
-  }
-  const int st_max = v3 ? 6 : 2;   // variant 4: every lane copies one chunk ahead of its reads: two stages
-  if (st > st_max) st = st_max;
-  if (h->opt_stages > 0 && h->opt_stages < st) st = h->opt_stages;
-  if (st < 2) st = 2;
-  if (!v3 && h->opt_window == 0 && acc_row_stride(w) <= N) w = acc_row_stride(w);   // the padding columns of a row are free
+  while (w > 1 && smem(G, w, 0) + st * stage > budget) --w;
+  if (h->opt_window == 0 && acc_row_stride(w) <= N) w = acc_row_stride(w);   // the padding columns of a row are free
   h->ws_W = w;
   h->ws_stages = st;
   int b = 1;
-  cudaError_t e = v3 ? acc_ws3_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b) : acc_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b);
+  cudaError_t e = acc_blocks_per_sm(G, w, ncw, pt, h->opt_il, st, &b);
   h->ws_blocks_per_sm = b > 0 ? b : 1;
   return e;
 }
@@ -329,7 +312,7 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.T64 = reinterpret_cast<double2*>(h->ws + h->lay.t64_off);
   p.counters = counters(h);
   const int blocks = acc_blocks(h);
-  const int ch = h->opt_variant == 3 ? acc_ws3_chunk(h->opt_ncw, h->opt_pt) : acc_chunk(h->opt_ncw, h->opt_pt);
+  const int ch = acc_chunk(h->opt_ncw, h->opt_pt);
   unsigned long long sc = (unsigned long long)h->opt_superchunk;
   if (sc == 0) {
     // aim at >= 8 scheduling units per block, between one chunk and 16K scatterers
@@ -347,7 +330,6 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   p.row_words = acc_row_stride(p.W);
   p.plane_words = acc_plane_words(h->cfg.n_gates, p.W);
   p.stages = h->ws_stages;
-  p.wait_hint = (unsigned)h->opt_wait_hint;
   {  // epoch of L scatterers: L adds of at most 2^fx_cap (+ rounding) per cell stay below 2^31
     const int L = ec * ch;
     int lg = 0;
@@ -385,23 +367,21 @@ int check_geometry(sim_handle* h, const sim_sat_state* sat) {
   return SIM_OK;
 }
 
-// One accumulation launch into the fp64 accumulator (variants 0, 4) or straight into T (variant 3).
+// One accumulation launch into the fp64 accumulator.
 int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_state* sat, float2* T) {
   AccParams p = make_acc_params(h, d_scat, sat, T);
   const int blocks = acc_blocks(h);
   int l = 0;
-  cudaError_t e = h->opt_variant == 3   ? launch_accumulate_ws3(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, h->stream, &l)
-                  : h->opt_variant == 0 ? launch_reference(p, h->sm_count, h->stream, &l)
-                                        : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->ticket_dirty, h->stream, &l);
+  cudaError_t e = h->opt_variant == 0 ? launch_reference(p, h->sm_count, h->stream, &l)
+                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->ticket_dirty, h->stream, &l);
   h->launches += l;
   if (l) h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
 }
 
-// fp64 accumulator -> spectrum slot (assign, or add for SIM_ACC_APPEND); variant 3 has accumulated in place.
+// fp64 accumulator -> spectrum slot (assign, or add for SIM_ACC_APPEND).
 int do_finalize(sim_handle* h, float2* T, bool add) {
-  if (h->opt_variant == 3) return SIM_OK;
   int l = 0;
   cudaError_t e = launch_finalize(reinterpret_cast<double2*>(h->ws + h->lay.t64_off), T, h->cfg.n_gates * h->cfg.n_doppler, add,
                                   counters(h), h->stream, &l);
@@ -588,10 +568,6 @@ int sim_accumulate_update(sim_handle* h, const sim_scatterers* d_scat, const sim
   int rc = begin_update(h, d_scat, sat, flags, true, &T);
   if (rc) return rc;
   const bool append = (flags & SIM_ACC_APPEND) != 0;
-  if (h->opt_variant == 3 && !append) {   // variant 3 accumulates straight into the slot
-    cudaError_t e = cudaMemsetAsync(T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
-  }
   rc = do_accumulate(h, d_scat, sat, T);
   if (rc == SIM_OK) rc = do_finalize(h, T, append);
   if (rc) {   // nothing is committed: the update was not started (or, for APPEND, the slot keeps its earlier batches)
@@ -612,10 +588,6 @@ int sim_accumulate_update_host(sim_handle* h, const sim_scatterers* h_scat, cons
   int rc = begin_update(h, h_scat, sat, flags, false, &T);
   if (rc) return rc;
   const bool append = (flags & SIM_ACC_APPEND) != 0;
-  if (h->opt_variant == 3 && !append) {
-    cudaError_t e = cudaMemsetAsync(T, 0, (size_t)h->cfg.n_gates * h->cfg.n_doppler * sizeof(float2), h->stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(spectrum)");
-  }
   const uint64_t chunk = (uint64_t)h->cfg.host_stage_scatterers;
   const size_t arr_stride = h->lay.stage_buf_bytes / 7;  // bytes between staged arrays
   const float* src[7] = {h_scat->x, h_scat->y, h_scat->z, h_scat->vx, h_scat->vy, h_scat->vz, h_scat->s0dA};
@@ -804,9 +776,8 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   p.dbg_g0 = d_gate0;
   p.dbg_k = d_bin;
   int l = 0;
-  // the production kernel itself, exporting its indices instead of accumulating (variant 3: its own index kernel)
-  cudaError_t e = h->opt_variant == 3 ? launch_indices3(p, d_gate0, d_bin, h->sm_count, h->stream, &l)
-                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, true, h->stream, &l);
+  // the production kernel itself, exporting its indices instead of accumulating
+  cudaError_t e = launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, true, h->stream, &l);
   h->launches += l;
   h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
@@ -848,9 +819,7 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
   };
   switch (option) {
     case SIM_OPT_ACC_VARIANT: {
-      if (value != 0 && value != 3 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant");
-      if (value == 3 && (h->cfg.n_doppler & (h->cfg.n_doppler - 1)))
-        return fail(h, SIM_ERR_INVALID_ARG, "accumulation variant 3 needs a power-of-two n_doppler");
+      if (value != 0 && value != 4) return fail(h, SIM_ERR_INVALID_ARG, "unknown accumulation variant (0 = reference kernel, 4 = production kernel)");
       const int old = h->opt_variant;
       h->opt_variant = (int)value;
       variant_defaults(h);   // warps, per-lane count and epoch length: back to the defaults
@@ -901,8 +870,9 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       h->opt_epoch = (int)value;
       return SIM_OK;
     case SIM_OPT_ACC_STAGES:
-      if (value > 8 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "TMA ring depth: 0 (auto) or 2..8");
-      return replan(h->opt_stages, (int)value, "ring depth cannot be planned");
+      if (value > 8 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "ring depth: 0 (auto) or 2..8");
+      h->opt_stages = (int)value;   // (accepted for compatibility: the production kernel always uses two stages)
+      return SIM_OK;
     case SIM_OPT_GUARD_LSB:
       if (value < 1 || value > (1 << (kFracBits - 2))) return fail(h, SIM_ERR_INVALID_ARG, "guard must be in 1..2^18");
       h->opt_guard = (int)value;

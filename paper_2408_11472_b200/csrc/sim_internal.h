@@ -57,17 +57,16 @@ struct AccParams {
   int lut_nu, lut_nv;
   float lut_u0, lut_v0, lut_inv_du, lut_inv_dv;
   int G, N;
-  float2* T;              // spectrum of the current update, [G][N] (variant 3 accumulates into it directly)
-  double2* T64;           // fp64 accumulator [G][N] (variants 0, 4): zero between updates, rounded to T by the finalize kernel
+  float2* T;              // spectrum slot of the current update, [G][N] (written by the finalize kernel)
+  double2* T64;           // fp64 accumulator [G][N]: zero between updates, rounded to T by the finalize kernel
   int32_t *dbg_g0, *dbg_k;   // index export of the production kernel (sim_debug_indices)
   unsigned int* counters; // kNumCounters device words
   unsigned long long superchunk; // scatterers per scheduling unit (whole fixed-point epochs)
   int W;                  // Doppler bins of the shared-memory window
   int row_words, plane_words;   // production kernel: tile layout (accumulate.cu)
-  int stages, epoch_chunks;  // TMA ring depth; chunks per fixed-point epoch
+  int stages, epoch_chunks;  // stages of the copy ring (2); chunks per fixed-point epoch
   int fx_cap, fx_target;     // block floating point: |c| s <= 2^fx_cap admitted; gmean(|c|) s in [2^fx_target, 2^(fx_target+1))
   unsigned long long sc_stride;  // scheduling unit visited by ticket t is (t * sc_stride) mod n_units (coprime)
-  unsigned wait_hint;        // variant 3: suspend-time hint of the mbarrier waits in ns (0 = plain try_wait loop)
 };
 
 struct SynParams {
@@ -89,7 +88,7 @@ struct SynParams {
   int weight_mode;
 };
 
-// production kernel (accumulate.cu): ncw compute warps + 1 drain warp per block, pt scatterers per lane per chunk
+// production kernel (accumulate.cu): ncw warps per block, pt scatterers per lane per chunk, il in flight per lane
 int acc_chunk(int ncw, int pt);
 int acc_row_stride(int W);
 int acc_plane_words(int G, int W);
@@ -100,13 +99,6 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
                               int* launches);
 cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches);
 cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, unsigned int* counters, cudaStream_t st, int* launches);
-// round-1 production kernel, kept for A/B (accumulate_ws3.cu): producer warp + drain warp + ncw compute warps
-size_t acc_ws3_smem_bytes(int G, int W, int ncw, int pt, int stages);
-bool acc_ws3_supported(int ncw, int pt, int il);
-cudaError_t acc_ws3_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
-cudaError_t launch_accumulate_ws3(const AccParams& p, int ncw, int pt, int il, int blocks, cudaStream_t st, int* launches);
-int acc_ws3_chunk(int ncw, int pt);
-cudaError_t launch_indices3(const AccParams& p, int32_t* g0, int32_t* k, int sm_count, cudaStream_t st, int* launches);
 // regular mode (regular.cu): Y[n_pulses][G] += per-pulse coherent sums; cudaErrorInvalidConfiguration when G is too
 // large for one pulse row per thread in shared memory
 cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,
