@@ -20,19 +20,19 @@ def pattern(nu, nv, half_u, half_v, alpha):
     return g.astype(np.complex64), u0, du, v0, dv
 
 
-def run(sim_mod, orc, wl, tab, u0, du, v0, dv, sat_kw=None, variants=(0, 4), tol=U.TOL):
+def run(sim_mod, orc, wl, tab, u0, du, v0, dv, sat_kw=None, variants=(0, 4), tol=U.TOL, doppler_mode=0):
     scat = W.scatterers(wl)
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     st = W.sat_state(wl, 0)
     st.update(sat_kw or {})
     sat_o = orc.make_sat(st["pos"], st["vel"], st["boresight"], st["range_gate0_m"])
     sat_g = sim_mod.make_sat(st["pos"], st["vel"], st["boresight"], st["range_gate0_m"])
-    T_ref = orc.spectrum_lut(U.oracle_cfg(orc, wl), sat_o, tab, u0, du, v0, dv, *[scat_np[f] for f in W.FIELDS],
+    T_ref = orc.spectrum_lut(U.oracle_cfg(orc, wl, doppler_mode=doppler_mode), sat_o, tab, u0, du, v0, dv, *[scat_np[f] for f in W.FIELDS],
                              nthreads=orc.max_threads())
     assert np.abs(T_ref).max() > 0
     worst = 0.0
     for variant in variants:
-        sim = sim_mod.Sim(sim_mod.config_for(wl))
+        sim = sim_mod.Sim(sim_mod.config_for(wl, doppler_mode=doppler_mode))
         sim.set_option(sim_mod.OPT_ACC_VARIANT, variant)
         sim.set_antenna_lut(torch.from_numpy(tab).cuda(), u0, du, v0, dv)
         sim.accumulate_update(scat_cuda, sat_g)
@@ -44,7 +44,7 @@ def run(sim_mod, orc, wl, tab, u0, du, v0, dv, sat_kw=None, variants=(0, 4), tol
         sim.set_antenna_lut(None)
         sim.accumulate_update(scat_cuda, sat_g)
         T_an = sim.get_spectrum(1).cpu().numpy()
-        T_an_ref = U.oracle_spectra(orc, wl, scat_np, [0])[0] if not sat_kw else None
+        T_an_ref = U.oracle_spectra(orc, wl, scat_np, [0], doppler_mode=doppler_mode)[0] if not sat_kw else None
         if T_an_ref is not None:
             assert U.rel_l2(T_an, T_an_ref) <= U.TOL
     return worst
@@ -70,6 +70,12 @@ def test_lut_nadir_patch_off_nadir_boresight_and_tilted_velocity(oracle, sim_mod
     wl = W.get("nadir_patch_16m").scaled(n_along=1000, n_cross=1021, n_updates=2)
     tab, u0, du, v0, dv = pattern(129, 129, 0.004, 0.004, wl.antenna_alpha)
     run(sim_mod, oracle, wl, tab, u0, du, v0, dv, sat_kw={"boresight": (0.0012, -0.0007, -1.0), "vel": (6990.0, 120.0, -3.0)})
+
+
+def test_lut_with_pulse_pair_doppler(oracle, sim_mod):
+    wl = W.get("nadir_patch_16m").scaled(n_along=600, n_cross=700, n_updates=2)
+    tab, u0, du, v0, dv = pattern(129, 97, 0.004, 0.004, wl.antenna_alpha)
+    run(sim_mod, oracle, wl, tab, u0, du, v0, dv, doppler_mode=1)
 
 
 def test_lut_partly_outside_the_recorded_pattern(oracle, sim_mod):

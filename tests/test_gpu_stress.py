@@ -1,6 +1,6 @@
 """Randomised (seeded) sweep over scene shapes, sizes, Doppler modes and every tuning knob of the production
 accumulation kernel: each draw must match the oracle (rel L2 <= 1e-4) and, above all, terminate: the kernel's
-compute and drain warps talk through mbarriers and shared-memory counters only, so a missed arrival would hang, not fail."""
+warps talk through mbarriers and shared-memory counters only, so a missed arrival would hang, not fail."""
 import random
 
 import numpy as np
@@ -24,7 +24,7 @@ def test_random_shapes_and_options(oracle, seed):
     rnd = random.Random(seed)
     for trial in range(40):
         G = rnd.choice([1, 7, 64, 128, 300])
-        N = rnd.choice([16, 64, 256, 2048])
+        N = rnd.choice([16, 64, 256, 2048, 48, 250, 1000])   # powers of two and mixed-radix sizes (bins are taken mod N)
         na, nc = rnd.randint(1, 300), rnd.randint(1, 400)
         sea = rnd.choice(["white", "white", "pm"]) if na >= 8 and nc >= 8 else "white"
         wl = W.get("tiny").scaled(n_along=na, n_cross=nc, n_gates=G, n_doppler=N, pulses_per_update=N, n_updates=1,
