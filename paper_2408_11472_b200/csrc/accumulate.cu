@@ -203,8 +203,6 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   const unsigned slice_lo = (unsigned)warp * SL;       // the warp's slice in a chunk
   const unsigned lane_smem = stage0 + (slice_lo + e0) * 4u;   // this lane's PT scatterers in stage 0, array 0
 
-  if (!DBG)
-    for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
   for (int i = tid; i < kRing; i += NCW * 32) sh::st(ut.seq0 + 4u * i, 0);
   if (tid < 4) sh::st(slot0 + 4u * kSlotInts * tid + 4 * kSlotState, kSlotUnset);
   if (tid < 2) {
@@ -214,14 +212,15 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     sh::mbar_fence_init();
   }
   __syncthreads();
-  if (tid == 0) {   // the first `ahead` units
+  if (tid == 0) {   // the first `ahead` units are static (tickets b and b + grid of block b): no round trip to the counter
     sh::st(claimed_a, 0);
     for (unsigned u = 0; u < ahead; ++u) {
-      PendingUnit t{atomicAdd(&p.counters[kCtrTicket], 1u), u, true};
+      PendingUnit t{blockIdx.x + u * gridDim.x, u, true};
       publish_unit(p, ut, n_sc, t);
     }
   }
   __syncthreads();
+  const unsigned ticket0 = ahead * gridDim.x;   // the counter hands out the tickets after the static ones
 
   PendingUnit tk{0u, 0u, false};
   // This lane's PT scatterers of the next chunk of the copy stream (7 x 16 bytes) -> its place in stage `st`; one commit
@@ -242,7 +241,8 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       // the first warp to enter a unit (index cs.unit - 1) prepares a later one
       if (!cs.stop) {
         if (lane == 0 && sh::cas(claimed_a, (int)cs.unit - 1, (int)cs.unit) == (int)cs.unit - 1) {
-          tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u);   // in flight until the end of this chunk
+          publish_unit(p, ut, n_sc, tk);   // (units of a single chunk: this warp's previous ticket may still be pending)
+          tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u) + ticket0;   // in flight until the end of this chunk
           tk.unit = cs.unit - 1u + ahead;
           tk.pending = true;
         }
@@ -274,6 +274,10 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   rd_base = cp_base;
   rd_nv = cp_nv;
   rd_first = cp_first;
+  if (!DBG) {   // the tiles are zeroed while the first chunk is on its way
+    for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
+    __syncthreads();
+  }
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
