@@ -32,7 +32,7 @@ extern "C" {
 
 #define SIM_OK 0
 #define SIM_ERR_INVALID_ARG (-1) /* NULL pointer, negative count, misaligned array, bad flag */
-#define SIM_ERR_BAD_CONFIG (-2)  /* sizes out of range, N not a power of two, non-positive lambda/PRF/dR */
+#define SIM_ERR_BAD_CONFIG (-2)  /* sizes out of range, N with a prime factor other than 2, 3, 5, non-positive lambda/PRF/dR */
 #define SIM_ERR_WORKSPACE (-3)   /* workspace too small or not 256-byte aligned */
 #define SIM_ERR_NOT_READY (-4)   /* synthesis needs a spectrum that has not been accumulated */
 #define SIM_ERR_OVERFLOW (-5)    /* more pending spectra than max_pending_updates */
