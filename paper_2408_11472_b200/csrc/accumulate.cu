@@ -87,12 +87,15 @@ struct UnitTable {
   unsigned start0, end0, seq0;   // shared-memory addresses of the three rings
 };
 
-__device__ __forceinline__ void publish_unit(const AccParams& p, const UnitTable& ut, unsigned long long n_sc, PendingUnit& t) {
+__device__ __forceinline__ void publish_unit(const AccParams& p, const UnitTable& ut, PendingUnit& t) {
   if (t.pending) {
     unsigned long long start = 0, end = 0;   // beyond the last ticket: an empty unit = end of work
-    if (t.ticket < n_sc) {
-      start = (((unsigned long long)t.ticket * p.sc_stride) % n_sc) * p.superchunk;   // tickets visit the scene in a scattered order
-      end = (start + p.superchunk < p.n) ? start + p.superchunk : p.n;
+    if (t.ticket < p.n_big) {                // whole units, visited in a scattered order
+      start = (((unsigned long long)t.ticket * p.sc_stride) % p.n_big) * p.superchunk;
+      end = start + p.superchunk;
+    } else if (t.ticket < p.n_units) {       // the last round: shorter units, in input order
+      start = p.tail_start + (unsigned long long)(t.ticket - p.n_big) * p.sc_small;
+      end = (start + p.sc_small < p.n) ? start + p.sc_small : p.n;
     }
     const unsigned slot = t.unit & (kRing - 1);
     sh::st64(ut.start0 + 8u * slot, start);
@@ -198,7 +201,6 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   // the copies run one chunk ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
   // need before the end of the chunk in which it is published
   const unsigned ahead = 2u;   // (two stages: the copies are one chunk ahead of the reads, at most one unit ahead)
-  const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
   const unsigned e0 = (unsigned)lane * PT;             // this lane's first scatterer in the warp's slice
   const unsigned slice_lo = (unsigned)warp * SL;       // the warp's slice in a chunk
   const unsigned lane_smem = stage0 + (slice_lo + e0) * 4u;   // this lane's PT scatterers in stage 0, array 0
@@ -216,7 +218,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     sh::st(claimed_a, 0);
     for (unsigned u = 0; u < ahead; ++u) {
       PendingUnit t{blockIdx.x + u * gridDim.x, u, true};
-      publish_unit(p, ut, n_sc, t);
+      publish_unit(p, ut, t);
     }
   }
   __syncthreads();
@@ -241,7 +243,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       // the first warp to enter a unit (index cs.unit - 1) prepares a later one
       if (!cs.stop) {
         if (lane == 0 && sh::cas(claimed_a, (int)cs.unit - 1, (int)cs.unit) == (int)cs.unit - 1) {
-          publish_unit(p, ut, n_sc, tk);   // (units of a single chunk: this warp's previous ticket may still be pending)
+          publish_unit(p, ut, tk);   // (units of a single chunk: this warp's previous ticket may still be pending)
           tk.ticket = atomicAdd(&p.counters[kCtrTicket], 1u) + ticket0;   // in flight until the end of this chunk
           tk.unit = cs.unit - 1u + ahead;
           tk.pending = true;
@@ -639,7 +641,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       }
       // the ticket drawn when this warp was first into a unit (at the top of this chunk) has had the whole chunk to come
       // back: the unit is published before this warp can wait for anybody
-      if (lane == 0) publish_unit(p, ut, n_sc, tk);
+      if (lane == 0) publish_unit(p, ut, tk);
       __syncwarp();
     }
 
@@ -651,7 +653,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       if (!more) try_drain(e + 1u, true);   // the end of the input: the shares of the last epochs
     }
   }
-  if (lane == 0) publish_unit(p, ut, n_sc, tk);
+  if (lane == 0) publish_unit(p, ut, tk);
   if (escapes) atomicAdd(&p.counters[kCtrEscape], escapes);
   if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
 }
@@ -763,8 +765,7 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
     e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) return e;
   }
-  const unsigned long long n_sc = (p.n + p.superchunk - 1) / p.superchunk;
-  const int grid = (int)(n_sc < (unsigned long long)blocks ? n_sc : (unsigned long long)blocks);
+  const int grid = (int)(p.n_units < (unsigned)blocks ? p.n_units : (unsigned)blocks);
   k<<<grid, ncw * 32, smem, st>>>(p);
   ++*launches;
   return cudaGetLastError();

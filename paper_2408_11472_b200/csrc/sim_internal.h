@@ -62,6 +62,10 @@ struct AccParams {
   int32_t *dbg_g0, *dbg_k;   // index export of the production kernel (sim_debug_indices)
   unsigned int* counters; // kNumCounters device words
   unsigned long long superchunk; // scatterers per scheduling unit (whole fixed-point epochs)
+  // tickets < n_big: whole units of `superchunk` in the scattered order; then the rest of the input, [tail_start, n), in
+  // shorter units of `sc_small` in input order (the last round: blocks finish closer together); n_units in all
+  unsigned n_big, n_units;
+  unsigned long long tail_start, sc_small;
   int W;                  // Doppler bins of the shared-memory window
   int row_words, plane_words;   // production kernel: tile layout (accumulate.cu)
   int stages, epoch_chunks;  // stages of the copy ring (2); chunks per fixed-point epoch
