@@ -342,7 +342,7 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
   if (sc > (1ull << 30)) sc = 1ull << 30;   // the kernels count the scatterers of a unit in 32 bits
   sc = (sc + unit - 1) / unit * unit;
   p.superchunk = sc;
-  {  // The last round of work goes in shorter units (a third of an epoch), in input order: the blocks then finish within
+  {  // The last round of work goes in shorter units (half an epoch), in input order: the blocks then finish within
      // a short unit of each other instead of a long one (measured on the 16.8M patch: the tail of a launch was about half
      // a unit, 7 us of 121).  Not when the caller fixed the unit size, and never more than a quarter of the input.
     const unsigned long long n_full = s->n / sc;
@@ -351,7 +351,7 @@ AccParams make_acc_params(sim_handle* h, const sim_scatterers* s, const sim_sat_
       tail_big = (unsigned long long)blocks < n_full / 4 ? (unsigned long long)blocks : n_full / 4;
     }
     const unsigned long long n_big = n_full - tail_big;
-    const int ec_small = tail_big ? (ec + 2) / 3 : ec;
+    const int ec_small = tail_big ? (ec + 1) / 2 : ec;   // (half, a third or a quarter of an epoch, and one round or two, measure alike within 1-2 %)
     p.sc_small = tail_big ? (unsigned long long)ch * ec_small : sc;
     p.tail_start = n_big * sc;
     const unsigned long long n_small = (s->n - p.tail_start + p.sc_small - 1) / p.sc_small;
