@@ -35,6 +35,7 @@
 // `sim_debug_indices` runs the production kernel itself with DBG = true (same index flow, indices written instead of
 // amplitudes accumulated).
 #include <climits>
+#include <cstdlib>
 
 #include "ptx_util.cuh"
 #include "scatter_math.cuh"
@@ -280,6 +281,10 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
     __syncthreads();
   }
+  // everything up to here touched only the inputs and shared memory: the launch may have started while the finalize
+  // kernel of the previous update was still running (programmatic dependent launch); the accumulator and the ticket
+  // counter are its to use from here on
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
@@ -656,6 +661,13 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   if (lane == 0) publish_unit(p, ut, tk);
   if (escapes) atomicAdd(&p.counters[kCtrEscape], escapes);
   if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
+  // the last block out leaves the scheduling counter at zero for the next launch (every block has drawn its last ticket
+  // before it gets here), so that the next launch may draw tickets before the finalize kernel in between has run
+  __syncthreads();
+  if (tid == 0 && atomicAdd(&p.counters[kCtrDone], 1u) == gridDim.x - 1u) {
+    p.counters[kCtrDone] = 0u;
+    p.counters[kCtrTicket] = 0u;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -680,10 +692,11 @@ __global__ void __launch_bounds__(256) acc_reference_kernel(AccParams p) {
 
 // T64 -> spectrum slot (complex64), T64 re-zeroed.  add != 0: the slot already holds earlier batches of this update
 // (SIM_ACC_APPEND).
-__global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add,
-                                                           unsigned int* __restrict__ counters) {
+__global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add) {
+  // the next accumulation launch may start now: it reads only its inputs and shared memory before it waits for this
+  // grid to complete (programmatic dependent launch; see acc_kernel)
+  asm volatile("griddepcontrol.launch_dependents;");
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) counters[kCtrTicket] = 0u;   // the scheduling counter of the next accumulation launch
   if (i >= cells) return;
   const double2 v = T64[i];
   float2 o = make_float2((float)v.x, (float)v.y);
@@ -696,8 +709,8 @@ __global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__
   if (v.x != 0.0 || v.y != 0.0) T64[i] = make_double2(0.0, 0.0);
 }
 
-cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, unsigned int* counters, cudaStream_t st, int* launches) {
-  acc_finalize_kernel<<<(cells + 255) / 256, 256, 0, st>>>(T64, T, cells, add ? 1 : 0, counters);
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches) {
+  acc_finalize_kernel<<<(cells + 255) / 256, 256, 0, st>>>(T64, T, cells, add ? 1 : 0);
   ++*launches;
   return cudaGetLastError();
 }
@@ -751,8 +764,7 @@ cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages,
 }
 
 // dbg: the same kernel writes (g0, k) per scatterer into p.dbg_g0 / p.dbg_k instead of accumulating.
-cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, bool reset_ticket, cudaStream_t st,
-                              int* launches) {
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches) {
   if (p.n == 0) return cudaSuccess;
   const int mode = acc_index_mode(p);
   AccKernel k = acc_kernel_ptr(ncw, pt, il, mode, dbg ? 2 : (p.lut != nullptr ? 1 : 0));
@@ -761,14 +773,23 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
   // per launch: the limit is per function and per device, another handle may have set it for a smaller shape
   cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  if (reset_ticket) {   // (the finalize kernel leaves the scheduling counter at zero: only needed when none ran in between)
-    e = cudaMemsetAsync(p.counters + kCtrTicket, 0, sizeof(unsigned int), st);
-    if (e != cudaSuccess) return e;
-  }
   const int grid = (int)(p.n_units < (unsigned)blocks ? p.n_units : (unsigned)blocks);
-  k<<<grid, ncw * 32, smem, st>>>(p);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(ncw * 32);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  // programmatic dependent launch: when the kernel before this one in the stream is the finalize kernel of the previous
+  // update (the only one that signals it), this grid may start while that one runs; it waits for it before it touches
+  // the accumulator (griddepcontrol.wait in acc_kernel).  After any other kernel the launch is serialised as usual.
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  e = cudaLaunchKernelEx(&cfg, k, p);
   ++*launches;
-  return cudaGetLastError();
+  return e;
 }
 
 cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches) {

@@ -98,7 +98,6 @@ struct sim_handle {
   int lut_nu, lut_nv;
   double lut_u0, lut_du, lut_v0, lut_dv;
   uint64_t launches, scatterers_seen;
-  bool ticket_dirty;             // the scheduling counter may be non-zero (an accumulation launch without a finalize after it)
   std::string err;
 };
 
@@ -387,9 +386,8 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
   const int blocks = acc_blocks(h);
   int l = 0;
   cudaError_t e = h->opt_variant == 0 ? launch_reference(p, h->sm_count, h->stream, &l)
-                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->ticket_dirty, h->stream, &l);
+                                      : launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, blocks, false, h->stream, &l);
   h->launches += l;
-  if (l) h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "accumulate launch");
   return SIM_OK;
 }
@@ -398,10 +396,9 @@ int do_accumulate(sim_handle* h, const sim_scatterers* d_scat, const sim_sat_sta
 int do_finalize(sim_handle* h, float2* T, bool add) {
   int l = 0;
   cudaError_t e = launch_finalize(reinterpret_cast<double2*>(h->ws + h->lay.t64_off), T, h->cfg.n_gates * h->cfg.n_doppler, add,
-                                  counters(h), h->stream, &l);
+                                  h->stream, &l);
   h->launches += l;
   if (e != cudaSuccess) return cuda_fail(h, e, "finalize launch");
-  h->ticket_dirty = false;
   return SIM_OK;
 }
 
@@ -541,7 +538,6 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->ws_blocks_per_sm = 0;
   h->launches = 0;
   h->scatterers_seen = 0;
-  h->ticket_dirty = true;
   int v = 0;
   e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cfg->device);
   if (e != cudaSuccess) { sim_destroy(h); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)"); }
@@ -791,9 +787,8 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
   p.dbg_k = d_bin;
   int l = 0;
   // the production kernel itself, exporting its indices instead of accumulating
-  cudaError_t e = launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, true, h->stream, &l);
+  cudaError_t e = launch_accumulate(p, h->opt_ncw, h->opt_pt, h->opt_il, acc_blocks(h), true, h->stream, &l);
   h->launches += l;
-  h->ticket_dirty = true;
   if (e != cudaSuccess) return cuda_fail(h, e, "indices launch");
   return SIM_OK;
 }

@@ -14,7 +14,7 @@ constexpr int kFracBits = 20;                 // fixed-point fraction bits of th
 enum Counter : int {
   kCtrTicket = 0,   // scheduling ticket of the running accumulation launch
   kCtrEscape = 1,   // contributions sent to global reductions (guard band, outside the window or the fixed-point range)
-  kCtrUnused = 2,
+  kCtrDone = 2,     // blocks of the running accumulation launch that have finished (the last one out resets the ticket)
   kCtrFallback = 3, // scatterers whose indices were decided by the canonical sequence (guard band)
 };
 
@@ -99,10 +99,9 @@ int acc_plane_words(int G, int W);
 size_t acc_smem_bytes(int G, int W, int ncw, int pt, int stages);
 bool acc_supported(int ncw, int pt, int il);
 cudaError_t acc_blocks_per_sm(int G, int W, int ncw, int pt, int il, int stages, int* blocks);
-cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, bool reset_ticket, cudaStream_t st,
-                              int* launches);
+cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int blocks, bool dbg, cudaStream_t st, int* launches);
 cudaError_t launch_reference(const AccParams& p, int sm_count, cudaStream_t st, int* launches);
-cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, unsigned int* counters, cudaStream_t st, int* launches);
+cudaError_t launch_finalize(double2* T64, float2* T, int cells, bool add, cudaStream_t st, int* launches);
 // regular mode (regular.cu): Y[n_pulses][G] += per-pulse coherent sums; cudaErrorInvalidConfiguration when G is too
 // large for one pulse row per thread in shared memory
 cudaError_t launch_regular(const AccParams& a, float2* Y, long long j0, int n_pulses, double prf, int sm_count,
