@@ -42,8 +42,6 @@
 
 namespace simk {
 
-constexpr int kAccMaxStages = 8;
-constexpr int kAccMaxWarps = 16;
 constexpr int kRing = 128;   // chunk table entries: more than two epochs (<= 2 * 31 chunks) + the stage ring
 
 // epoch parameter slot (ring of 4): state, first bin of the Doppler window (unwrapped), scale exponent
@@ -198,7 +196,6 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   const unsigned complete0 = sh::addr(&s_bar_complete[0]), drained0 = sh::addr(&s_bar_drained[0]);
   const unsigned shares0 = sh::addr(&s_shares[0]);
   const unsigned slot0 = sh::addr(&s_slot[0][0]);
-  const unsigned cps = (unsigned)(p.superchunk / CH);          // chunks per scheduling unit
   // the copies run one chunk ahead of the reads: entering unit u, a warp prepares unit u + ahead, which no copy can
   // need before the end of the chunk in which it is published
   const unsigned ahead = 2u;   // (two stages: the copies are one chunk ahead of the reads, at most one unit ahead)
