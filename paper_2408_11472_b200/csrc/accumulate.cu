@@ -60,8 +60,12 @@ int acc_row_stride(int W) {
   while ((rs & 7) != 4) rs += 2;
   return rs;
 }
+// Rows of a plane: G + 1 gate rows, then enough rows to give every lane of a warp its own "dump" word, where the
+// reductions of a scatterer that the tile cannot take are sent (never read, never zeroed): the four reductions are
+// issued unconditionally, without a branch around them.
+static int acc_dump_rows(int W) { return (32 + acc_row_stride(W) - 1) / acc_row_stride(W); }
 int acc_plane_words(int G, int W) {
-  int w = (G + 1) * acc_row_stride(W);
+  int w = (G + 1 + acc_dump_rows(W)) * acc_row_stride(W);
   while ((w & 31) != 2) w += 2;
   return w;
 }
@@ -372,6 +376,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     // tile base of this lane's first reduction, the +1 row offset of the padded tile folded in
     unsigned tile_b = tile0 + (e & 1u) * tile_bytes + off_b0;
     asm volatile("" : "+r"(tile_b));
+    const unsigned dump_b = tile_b + (unsigned)(G * RS4 + 4 * lane);   // row G + 1 onwards of this lane's first plane
     bool have = false;         // this warp holds the epoch's parameters
     int k0 = 0, lo_bits = 0;
     float s = 0.0f, sS = 0.0f, sO = 0.0f;
@@ -601,13 +606,11 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
         for (int j = 0; j < IL; ++j) {
           const int kw = k[j] - k0;
           const bool fits = ok[j] && !near[j] && (unsigned)kw < (unsigned)W && (unsigned)(ab[j] - lo_bits) <= fx_span;
-          const unsigned adr = tile_b + (unsigned)(g0[j] * RS4 + 4 * kw);
-          if (fits) {
-            sh::red_add(adr, r0[j]);
-            sh::red_add(adr + d_ri, r1[j]);
-            sh::red_add(adr + d_lu, r2[j]);
-            sh::red_add(adr + d_lu + d_ri, r3[j]);
-          }
+          const unsigned adr = fits ? tile_b + (unsigned)(g0[j] * RS4 + 4 * kw) : dump_b;   // (tile cell, or this lane's dump word)
+          sh::red_add(adr, r0[j]);
+          sh::red_add(adr + d_ri, r1[j]);
+          sh::red_add(adr + d_lu, r2[j]);
+          sh::red_add(adr + d_lu + d_ri, r3[j]);
           slow[j] = ok[j] && !fits;
           slow_any |= slow[j];
         }
