@@ -282,9 +282,9 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
     __syncthreads();
   }
-  // everything up to here touched only the inputs and shared memory: the launch may have started while the finalize
-  // kernel of the previous update was still running (programmatic dependent launch); the accumulator and the ticket
-  // counter are its to use from here on
+  // everything up to here touched only the inputs, shared memory and the ticket counter (left at zero by the last block
+  // of the previous accumulation launch): the launch may have started while the finalize kernel of the previous update
+  // was still running (programmatic dependent launch); the accumulator is its to use from here on
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
