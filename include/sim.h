@@ -230,6 +230,43 @@ int sim_get_stats(const sim_handle* h, sim_stats* out);
  * reset != 0, zeroes them. */
 int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset);
 
+/* ---- one update without any device allocation by anybody ------------------------------------------ */
+
+/* Every call above needs a device workspace, and somebody has to allocate it.  Some users of this library cannot:
+ * a radar-chain plug-in running inside a host simulator that took the whole device for its own arena at start-up and
+ * hands plug-ins nothing but their input and output buffers; a processing loop with a latency bound, where
+ * cudaMalloc / cudaFree would stall every stream of the device; a process held to a device-memory quota that is
+ * already spent.  sim_accumulate_static is steps A1-A7 (the same production accumulation kernel and the same
+ * finalize kernel as sim_accumulate_update) for ONE update with no handle and no workspace: the
+ * fp64 accumulator and the scheduling counters of the kernel live in a fixed array compiled into libsim.so
+ * (SIM_STATIC_MAX_CELLS fp64 pairs = 1 MiB, plus 256 bytes of counters; every GPU on which the library is used holds
+ * that much until the process exits).  The call itself allocates nothing: no cudaMalloc, no cudaFree, no library
+ * routine that allocates.
+ *
+ *   cfg         HOST.  n_gates, n_doppler, wavelength_m, prf_hz, gate_spacing_m, antenna_alpha, doppler_mode and device
+ *               are used; the other fields must merely be valid (see sim_config).  n_gates * n_doppler must not exceed
+ *               SIM_STATIC_MAX_CELLS (all five BASELINE configs fit: 128 x 512 at most): SIM_ERR_BAD_CONFIG otherwise.
+ *   d_scat      DEVICE arrays as for sim_accumulate_update (16-byte aligned; n may be 0).
+ *   sat         HOST, read during the call.
+ *   d_spectrum  DEVICE, complex64 [n_gates][n_doppler], bin fastest, 16-byte aligned, owned by the caller.
+ *               flags = 0: overwritten with the update's spectrum.  flags = SIM_ACC_APPEND: the batch is added to what
+ *               it holds (scenes delivered in pieces).
+ *   cuda_stream a cudaStream_t on cfg->device (NULL = legacy default stream); the work is enqueued, not waited for.
+ *
+ * The analytic antenna gain only (a tabulated pattern belongs to a handle).
+ * First call on a device: the library looks up the device address of its array and reads three device attributes
+ * (once per device, kept for later calls), and the CUDA runtime loads the kernels.  Make that first call during
+ * start-up, outside any stream capture.
+ * The array is shared by every call in the process.  Each call clears the part it uses before the kernel runs, so
+ * nothing is carried over from the call before; but two calls whose GPU work overlaps in time (different streams, or
+ * different host threads on different streams) race on it and both results are garbage: keep all calls of a device
+ * on one stream, or order them with events.  Calls on different devices do not interact.
+ * Errors: SIM_ERR_INVALID_ARG (NULL / misaligned pointers, unknown flag), SIM_ERR_BAD_CONFIG (invalid cfg, too many
+ * cells, gate window too deep), SIM_ERR_CUDA.  Message: sim_last_error(NULL) on the calling thread. */
+#define SIM_STATIC_MAX_CELLS 65536
+int sim_accumulate_static(const sim_config* cfg, const sim_scatterers* d_scat, const sim_sat_state* sat,
+                          void* d_spectrum, void* cuda_stream, uint32_t flags);
+
 /* Message of the last error on this handle ("" if none); valid until the next call.  h may be NULL
  * (returns the message of the last failed sim_create / sim_workspace_bytes on this thread). */
 const char* sim_last_error(const sim_handle* h);

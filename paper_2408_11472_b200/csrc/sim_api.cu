@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -923,3 +924,124 @@ int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset) {
 const char* sim_last_error(const sim_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// sim_accumulate_static: one update for callers that have no device workspace and cannot get one (include/sim.h).
+// The scratch memory of the accumulation kernels -- the fp64 accumulator and the scheduling counters, which the other
+// entry points keep in the caller's workspace -- is this file-scope array instead.  It is part of the library image:
+// each device that runs anything from libsim.so holds one copy (zero-filled when the module is loaded) until exit.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kStaticAccBytes = (size_t)SIM_STATIC_MAX_CELLS * sizeof(double2);   // 1 MiB
+constexpr size_t kStaticCtrBytes = kNumCounters * sizeof(unsigned int);               // 256 B
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticAccBytes + kStaticCtrBytes];
+
+// What the first call on a device finds out, kept for the later ones.  In host code `g_static_scratch` is only a
+// stand-in for the symbol, not an address a kernel could use: the device address comes from cudaGetSymbolAddress,
+// asked for with that device current.
+struct StaticDevice {
+  bool ready = false;
+  unsigned char* scratch = nullptr;   // device address of g_static_scratch on this device
+  int sm_count = 0;
+  size_t smem_optin = 0, smem_per_sm = 0;
+};
+constexpr int kStaticMaxDevices = 64;
+StaticDevice g_static_device[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+// Caller has made `device` current.  No allocation: one symbol look-up and three attribute queries.
+int static_device(int device, StaticDevice* out) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticDevice& d = g_static_device[device];
+  if (!d.ready) {
+    void* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetSymbolAddress(static scratch)");
+    if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) return fail(nullptr, SIM_ERR_CUDA, "static scratch: unusable device address");
+    int v = 0;
+    e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(sm count)");
+    d.sm_count = v;
+    e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem optin)");
+    d.smem_optin = (size_t)v;
+    e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaDeviceGetAttribute(smem per SM)");
+    d.smem_per_sm = (size_t)v;
+    d.scratch = static_cast<unsigned char*>(ptr);
+    d.ready = true;
+  }
+  *out = d;
+  return SIM_OK;
+}
+
+}  // namespace
+
+extern "C" int sim_accumulate_static(const sim_config* cfg, const sim_scatterers* d_scat, const sim_sat_state* sat,
+                                     void* d_spectrum, void* cuda_stream, uint32_t flags) {
+  if (const char* m = check_config(cfg)) return fail(nullptr, cfg ? SIM_ERR_BAD_CONFIG : SIM_ERR_INVALID_ARG, m);
+  const size_t cells = (size_t)cfg->n_gates * (size_t)cfg->n_doppler;
+  if (cells > (size_t)SIM_STATIC_MAX_CELLS)
+    return fail(nullptr, SIM_ERR_BAD_CONFIG,
+                "sim_accumulate_static: n_gates * n_doppler = " + std::to_string(cells) + " exceeds SIM_STATIC_MAX_CELLS = " +
+                    std::to_string(SIM_STATIC_MAX_CELLS) + " (the built-in accumulator); use sim_create with a workspace");
+  if (flags & ~SIM_ACC_APPEND) return fail(nullptr, SIM_ERR_INVALID_ARG, "unknown accumulate flag");
+  if (!d_spectrum) return fail(nullptr, SIM_ERR_INVALID_ARG, "d_spectrum is NULL");
+  if (misaligned(d_spectrum)) return fail(nullptr, SIM_ERR_INVALID_ARG, "d_spectrum must be 16-byte aligned");
+  if (cfg->device >= kStaticMaxDevices) return fail(nullptr, SIM_ERR_BAD_CONFIG, "cfg.device beyond the devices this entry point keeps state for");
+  int n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount");
+  if (cfg->device >= n_dev) return fail(nullptr, SIM_ERR_BAD_CONFIG, "cfg.device is not a CUDA device of this process");
+  DeviceGuard guard(cfg->device);
+  StaticDevice dev;
+  int rc = static_device(cfg->device, &dev);
+  if (rc) return rc;
+
+  // A handle that lives on this stack frame only and owns nothing on the device: it carries the configuration and the
+  // default launch shape to the same planning and parameter code the handle-based calls use.
+  sim_handle t{};
+  t.cfg = *cfg;
+  t.cfg.host_stage_scatterers = 0;
+  t.cfg.host_stage_pulses = 0;
+  t.stream = static_cast<cudaStream_t>(cuda_stream);
+  t.sm_count = dev.sm_count;
+  t.smem_optin = dev.smem_optin;
+  t.smem_per_sm = dev.smem_per_sm;
+  t.opt_variant = 4;
+  variant_defaults(&t);
+  t.opt_scatter = 1;
+  t.opt_index_path = 1;
+  t.opt_guard = 16;
+  auto leave = [&](int code) {   // messages of the shared checks land in the temporary handle: hand them to the thread
+    if (code) g_create_error = t.err;
+    return code;
+  };
+  rc = check_scatterers(&t, d_scat, true);
+  if (rc) return leave(rc);
+  rc = check_sat(&t, sat);
+  if (rc) return leave(rc);
+  rc = check_geometry(&t, sat);
+  if (rc) return leave(rc);
+  e = plan_ws(&t);
+  if (e != cudaSuccess) return leave(cuda_fail(&t, e, "accumulation kernel occupancy query"));
+
+  float2* T = static_cast<float2*>(d_spectrum);
+  AccParams p = make_acc_params(&t, d_scat, sat, T);
+  p.T64 = reinterpret_cast<double2*>(dev.scratch);
+  p.counters = reinterpret_cast<unsigned int*>(dev.scratch + kStaticAccBytes);
+  // The array keeps what the last call left.  Counters first, accumulator second: the accumulation kernel may start
+  // under the tail of the operation just before it (programmatic dependent launch) and draws scheduling tickets before
+  // it waits for that operation; it touches the accumulator only after the wait.  So the operation just before it must
+  // be the accumulator's clear, with the counters' clear complete before that.
+  e = cudaMemsetAsync(p.counters, 0, kStaticCtrBytes, t.stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(p.T64, 0, cells * sizeof(double2), t.stream);
+  if (e != cudaSuccess) return leave(cuda_fail(&t, e, "cudaMemsetAsync(static scratch)"));
+  int l = 0;
+  e = launch_accumulate(p, t.opt_ncw, t.opt_pt, t.opt_il, acc_blocks(&t), false, t.stream, &l);
+  if (e != cudaSuccess) return leave(cuda_fail(&t, e, "accumulate launch"));
+  e = launch_finalize(p.T64, T, (int)cells, (flags & SIM_ACC_APPEND) != 0, t.stream, &l);
+  if (e != cudaSuccess) return leave(cuda_fail(&t, e, "finalize launch"));
+  return SIM_OK;
+}

@@ -29,7 +29,9 @@ EXPORTS = [
     "sim_accumulate_update_host", "sim_synthesize_pulses_host", "sim_synchronize", "sim_destroy",
     "sim_get_spectrum", "sim_spectrum_offset", "sim_debug_indices", "sim_set_option", "sim_get_stats",
     "sim_read_counters", "sim_last_error", "sim_regular_pulses", "sim_burst_beams", "sim_set_antenna_lut",
+    "sim_accumulate_static",
 ]
+STATIC_MAX_CELLS = 65536
 
 
 class SimError(RuntimeError):
@@ -93,6 +95,8 @@ def load_library(build_if_missing: bool = True):
     L.sim_set_antenna_lut.argtypes = [hp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double]
     L.sim_get_stats.argtypes = [hp, C.POINTER(SimStats)]
     L.sim_read_counters.argtypes = [hp, C.POINTER(C.c_uint32), C.c_int32]
+    L.sim_accumulate_static.argtypes = [C.POINTER(SimConfig), C.POINTER(SimScatterers), C.POINTER(SimSatState), vp, vp,
+                                        C.c_uint32]
     L.sim_last_error.argtypes = [hp]
     L.sim_last_error.restype = C.c_char_p
     for name in EXPORTS:
@@ -271,6 +275,30 @@ class Sim:
         a = (C.c_uint32 * 4)()
         self._check(self.lib.sim_read_counters(self._h, a, int(reset)), self._h)
         return {"tickets": a[0], "escapes": a[1], "flushes": a[2], "index_fallbacks": a[3]}
+
+
+def accumulate_static(cfg: SimConfig, scat: dict, sat: SimSatState, out: "torch.Tensor | None" = None,
+                      stream: "torch.cuda.Stream | None" = None, flags: int = 0) -> torch.Tensor:
+    """sim_accumulate_static: the spectrum [G][N] of one update, for callers that cannot provide a device workspace
+    (no handle; the kernel's scratch memory is an array built into libsim.so, G * N <= STATIC_MAX_CELLS).  `out` is
+    the caller's complex64 CUDA buffer; only when none is given does this wrapper ask torch for one, which a caller
+    that cannot allocate would not do.  Calls that overlap on the GPU share the scratch array and race."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2408_11472_b200.sim needs a CUDA device (B200); there is no CPU fallback")
+    lib = load_library()
+    device = torch.device("cuda", cfg.device)
+    if out is None:
+        out = torch.empty((cfg.n_gates, cfg.n_doppler), dtype=torch.complex64, device=device)
+    if out.dtype != torch.complex64 or not out.is_contiguous() or not out.is_cuda or out.numel() < cfg.n_gates * cfg.n_doppler:
+        raise ValueError("out must be a contiguous CUDA complex64 tensor of at least G*N elements")
+    s = _scat_struct(scat, cuda=True)
+    st = stream if stream is not None else torch.cuda.current_stream(device)
+    rc = lib.sim_accumulate_static(C.byref(cfg), C.byref(s), C.byref(sat), C.c_void_p(out.data_ptr()),
+                                   C.c_void_p(st.cuda_stream), C.c_uint32(flags))
+    if rc != OK:
+        msg = lib.sim_last_error(None)
+        raise SimError(rc, msg.decode() if msg else "")
+    return out
 
 
 def config_for(wl, **kw) -> SimConfig:
