@@ -16,6 +16,8 @@
  *     and (when host staging is enabled) one internal copy stream and a few events.
  *   - Every call enqueues work on the CUDA stream given to sim_create and returns without
  *     synchronising, unless stated.  Device inputs must stay valid until the stream reaches that point.
+ *     Stream order holds for them: whatever was enqueued earlier on that stream (a kernel of the caller's that writes
+ *     the scatterer arrays, say) is complete and visible before a kernel of the library reads them.
  *   - Every function returns SIM_OK or a negative SIM_ERR_*; nothing throws, nothing aborts.  After
  *     an error the handle is unchanged and still usable.  sim_last_error gives a message.
  *   - Not thread-safe per handle.  Distinct handles are independent.

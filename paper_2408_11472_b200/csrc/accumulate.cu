@@ -274,18 +274,20 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
     }
     sh::cp_async_commit();
   };
+  if (!DBG) {
+    for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
+    __syncthreads();
+  }
+  // Everything up to here touched shared memory only: the launch may have started while the kernel before it in the
+  // stream was still running (programmatic dependent launch: the finalize kernel of the previous update signals it
+  // early; behind any other kernel the launch is serialised as usual).  Nothing the caller owns and nothing in the
+  // workspace is read before this wait: a kernel of the caller's that writes the scatterer arrays earlier in the
+  // stream (a surface update) is complete and visible from here on, and so are the accumulator and the ticket counter.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   copy_chunk(0u);   // chunk 0 is in flight (two stages: the copies run one chunk ahead of the reads)
   rd_base = cp_base;
   rd_nv = cp_nv;
   rd_first = cp_first;
-  if (!DBG) {   // the tiles are zeroed while the first chunk is on its way
-    for (unsigned a = 4u * tid; a < 2u * tile_bytes; a += 4u * NCW * 32) sh::st(tile0 + a, 0);
-    __syncthreads();
-  }
-  // everything up to here touched only the inputs, shared memory and the ticket counter (left at zero by the last block
-  // of the previous accumulation launch): the launch may have started while the finalize kernel of the previous update
-  // was still running (programmatic dependent launch); the accumulator is its to use from here on
-  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // Step A7: this warp's share (gates [g_lo, g_hi)) of the tile of a completed epoch d -> T64, cells zeroed; the last
   // warp to finish its share hands the tile back.  Gate g = lower halves of row g + 1 (scatterers with g0 = g) + upper
@@ -662,7 +664,7 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
   if (escapes) atomicAdd(&p.counters[kCtrEscape], escapes);
   if (fallbacks) atomicAdd(&p.counters[kCtrFallback], fallbacks);
   // the last block out leaves the scheduling counter at zero for the next launch (every block has drawn its last ticket
-  // before it gets here), so that the next launch may draw tickets before the finalize kernel in between has run
+  // before it gets here): no memset between launches
   __syncthreads();
   if (tid == 0 && atomicAdd(&p.counters[kCtrDone], 1u) == gridDim.x - 1u) {
     p.counters[kCtrDone] = 0u;
@@ -693,8 +695,8 @@ __global__ void __launch_bounds__(256) acc_reference_kernel(AccParams p) {
 // T64 -> spectrum slot (complex64), T64 re-zeroed.  add != 0: the slot already holds earlier batches of this update
 // (SIM_ACC_APPEND).
 __global__ void __launch_bounds__(256) acc_finalize_kernel(double2* __restrict__ T64, float2* __restrict__ T, int cells, int add) {
-  // the next accumulation launch may start now: it reads only its inputs and shared memory before it waits for this
-  // grid to complete (programmatic dependent launch; see acc_kernel)
+  // the next accumulation launch may start now: it sets up its shared memory, then waits for this grid to complete
+  // before it reads anything from global memory (programmatic dependent launch; see acc_kernel)
   asm volatile("griddepcontrol.launch_dependents;");
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= cells) return;
@@ -782,8 +784,9 @@ cudaError_t launch_accumulate(const AccParams& p, int ncw, int pt, int il, int b
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   // programmatic dependent launch: when the kernel before this one in the stream is the finalize kernel of the previous
-  // update (the only one that signals it), this grid may start while that one runs; it waits for it before it touches
-  // the accumulator (griddepcontrol.wait in acc_kernel).  After any other kernel the launch is serialised as usual.
+  // update (the only one of ours that signals it), this grid may start while that one runs; it waits for it before it
+  // reads or writes any global memory (griddepcontrol.wait in acc_kernel), so stream order holds for the caller's
+  // arrays too, whatever kernel of the caller's comes before this one.
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;

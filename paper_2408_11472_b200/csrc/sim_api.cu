@@ -1031,10 +1031,9 @@ extern "C" int sim_accumulate_static(const sim_config* cfg, const sim_scatterers
   AccParams p = make_acc_params(&t, d_scat, sat, T);
   p.T64 = reinterpret_cast<double2*>(dev.scratch);
   p.counters = reinterpret_cast<unsigned int*>(dev.scratch + kStaticAccBytes);
-  // The array keeps what the last call left.  Counters first, accumulator second: the accumulation kernel may start
-  // under the tail of the operation just before it (programmatic dependent launch) and draws scheduling tickets before
-  // it waits for that operation; it touches the accumulator only after the wait.  So the operation just before it must
-  // be the accumulator's clear, with the counters' clear complete before that.
+  // The array keeps what the last call left: the scheduling counters and the cells this call uses start at zero.  (The
+  // accumulation kernel may start under the tail of the operation before it -- programmatic dependent launch -- but
+  // reads no global memory before it has waited for that operation, so both clears are complete when it looks.)
   e = cudaMemsetAsync(p.counters, 0, kStaticCtrBytes, t.stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(p.T64, 0, cells * sizeof(double2), t.stream);
   if (e != cudaSuccess) return leave(cuda_fail(&t, e, "cudaMemsetAsync(static scratch)"));
