@@ -303,9 +303,12 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
       const double inv_s = __hiloint2double((1023 - ex) << 20, 0);
       const unsigned tile = tile0 + b * tile_bytes;
       const int nitem = (g_hi - g_lo) * pairs;
-      const unsigned inv_pairs = (65536u + (unsigned)pairs - 1u) / (unsigned)pairs;   // it / pairs = (it * inv_pairs) >> 16 (it < 65536 / pairs)
+      // it / pairs = umulhi(it, ceil(2^32 / pairs)): exact while it < 2^32 / pairs (the error of the rounded-up reciprocal,
+      // < pairs * 2^-32 per unit of `it`, must stay below one): pairs <= 1026 (window option <= 2048) and nitem <=
+      // 129 * 1026 are far inside; pairs >= 2 (a row has at least four words) keeps the reciprocal in 32 bits
+      const unsigned inv_pairs = (unsigned)((0x100000000ull + (unsigned long long)pairs - 1ull) / (unsigned long long)pairs);
       for (int it = lane; it < nitem; it += 32) {
-        const int gi_ = (int)(((unsigned)it * inv_pairs) >> 16);
+        const int gi_ = (int)__umulhi((unsigned)it, inv_pairs);
         const int g = g_lo + gi_, q2 = (it - gi_ * pairs) * 2;
         const unsigned aL = tile + 4u * (unsigned)((g + 1) * RS + q2), aU = tile + 2u * plane_bytes + 4u * (unsigned)(g * RS + q2);
         const int2 lr = sh::ld2(aL), li = sh::ld2(aL + plane_bytes), ur = sh::ld2(aU), ui = sh::ld2(aU + plane_bytes);
@@ -371,6 +374,11 @@ __global__ void __launch_bounds__(NCW * 32, NCW <= 8 ? 2 : 1) acc_kernel(AccPara
 
   for (unsigned e = 0; more; ++e) {
     const unsigned slot = slot0 + 4u * kSlotInts * (e & 3u);
+    // The index export has no tiles and hence no tile hand-over to keep the warps of a block within two epochs of each
+    // other; without a bound a warp could run more than kRing units ahead of a sibling and overwrite unit-table entries
+    // the sibling has not read.  Every warp walks the same chunks and epochs (the stream is block-uniform), so a
+    // barrier per epoch is safe, and cheap enough for a debug path.
+    if (DBG) __syncthreads();
     if (!DBG && e >= 2) {   // the tile of epoch e-2 must be back: this warp's own share first, then everybody else's
       try_drain(e - 1u, true);
       sh::mbar_wait_sleepy(drained0 + 8u * (e & 1u), ((e >> 1) - 1u) & 1u, 2000u);

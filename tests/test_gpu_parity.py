@@ -271,6 +271,28 @@ def test_shuffled_order_and_tiny_window(oracle, sim_mod):
             assert sim.read_counters()["escapes"] > 0
 
 
+@pytest.mark.parametrize("G", [1, 2, 3, 4])
+def test_few_gates_wide_window(oracle, sim_mod, G):
+    """With very few gates the planner fits a window of several hundred Doppler bins into shared memory; the drain of
+    such a tile indexes (gate, bin pair) items far beyond the 16-bit range of the reciprocal division the drain used
+    up to round 2 (wrong cells for windows of 565 bins and more).  Velocities are scaled so that the
+    whole window is populated."""
+    wl = W.get("tiny").scaled(n_along=300, n_cross=301, n_gates=G, n_doppler=2048, pulses_per_update=2048, n_updates=1)
+    scat = W.scatterers(wl)
+    scat["vz"] *= 60.0
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
+    assert (np.abs(T_ref).max(axis=0) > 0).sum() > 800
+    for shape in ((8, 4, 4), (8, 2, 2)):
+        for window in (2048, 700, 566):
+            sim = sim_mod.Sim(sim_mod.config_for(wl))
+            sim.set_option(sim_mod.OPT_ACC_SHAPE, (shape[0] << 16) | (shape[1] << 8) | shape[2])
+            sim.set_option(sim_mod.OPT_ACC_WINDOW_BINS, window)
+            sim.accumulate_update(scat_cuda, sim_mod.sat_for(wl, 0))
+            e = U.rel_l2(sim.get_spectrum(0).cpu().numpy(), T_ref)
+            assert e <= U.TOL, (G, shape, window, e)
+
+
 def test_guard_band_and_exact_boundaries(oracle, sim_mod):
     """Fast index path: (i) scatterers sitting EXACTLY on gate boundaries and on Doppler-bin ties are
     decided by the canonical sequence (bit-exact indices); (ii) any guard width gives the same indices;
@@ -358,7 +380,7 @@ def test_block_shapes_and_epoch_lengths(oracle, sim_mod, ncw, pt, il):
     scat = W.scatterers(wl)
     scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
     T_ref = U.oracle_spectra(oracle, wl, scat_np, [0])[0]
-    for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 0}), (4095, {sim_mod.OPT_ACC_STAGES: 2, sim_mod.OPT_ACC_WINDOW_BINS: 11}),
+    for epoch, extra in ((1024, {}), (2047, {sim_mod.OPT_ACC_SCATTER: 0}), (4095, {sim_mod.OPT_ACC_WINDOW_BINS: 11}),
                          (8191, {sim_mod.OPT_ACC_SUPERCHUNK: 1}), (16383, {sim_mod.OPT_ACC_BLOCKS: 3})):
         sim = sim_mod.Sim(sim_mod.config_for(wl))
         sim.set_option(sim_mod.OPT_ACC_SHAPE, (ncw << 16) | (pt << 8) | il)
@@ -538,6 +560,22 @@ def test_paper_shaped_update_intervals(oracle, sim_mod, P, N):
         assert U.rel_l2(iq[s * P:(s + 1) * P], Y[s * P:(s + 1) * P]) <= U.TOL
     with pytest.raises(sim_mod.SimError):
         sim.synthesize_pulses(1)                                  # the next segment has no successor yet
+
+
+@pytest.mark.parametrize("N", [4096, 3072, 3125, 3750, 3600])
+def test_largest_accepted_doppler_sizes(oracle, sim_mod, N):
+    """sim_config admits n_doppler up to 4096 (the paper needs N = 2 n_fast = 2500 at most): the top of
+    the accepted range is run too -- a power of two, 3 * 2^10, 5^5, 2 * 3 * 5^4 and 2^4 3^2 5^2, P = N, 128 gates: spectra,
+    IQ per block, bin indices."""
+    wl = W.get("nadir_patch_16m").scaled(n_along=128, n_cross=200, n_gates=128, n_doppler=N, pulses_per_update=N,
+                                         n_updates=2)
+    scat = W.scatterers(wl)
+    scat["vz"] *= 25.0                                           # populate a few hundred bins
+    scat_np, scat_cuda = U.to_numpy(scat), U.to_cuda(scat)
+    T_ref = U.oracle_spectra(oracle, wl, scat_np, range(wl.n_updates))
+    T, iq, sim = U.gpu_run(sim_mod, wl, scat_cuda)
+    U.check_stream(oracle, wl, T, iq, T_ref)
+    _indices_exact(oracle, sim_mod, wl, scat_cuda, scat_np, sim, u=1)
 
 
 # ---- SURVEY.md 8(f) NEXT #4: Delay-Doppler burst step (PAPER.md:145-149) -------------------------------------
