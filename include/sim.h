@@ -211,10 +211,8 @@ int sim_debug_indices(sim_handle* h, const sim_scatterers* d_scat, const sim_sat
 #define SIM_OPT_ACC_WINDOW_BINS 4 /* Doppler bins held in shared memory; 0 = auto (as many as fit, up to 20) */
 #define SIM_OPT_GUARD_LSB 5     /* guard band of the fast index path in units of 2^-20 gate / bin (default 16) */
 #define SIM_OPT_ACC_WARPS 9      /* warps per block: 8 (default, two blocks per SM) or 16 */
-#define SIM_OPT_ACC_STAGES 10    /* accepted and ignored (the production kernel copies one chunk ahead: two stages) */
 #define SIM_OPT_ACC_PER_LANE 11  /* scatterers per lane per chunk: 2 or 4 (default) */
 #define SIM_OPT_ACC_EPOCH 12     /* scatterers per fixed-point epoch: 64..16383 (default 8191) */
-#define SIM_OPT_ACC_WAIT_HINT 13 /* accepted and ignored */
 #define SIM_OPT_ACC_SCATTER 14   /* 1 (default) = scheduling units visit the scene in a scattered order (dark and
                                     illuminated parts in flight together); 0 = in input order */
 #define SIM_OPT_ACC_INTERLEAVE 15 /* scatterers in flight per lane at a time: 2 or 4 (<= per lane) */
@@ -225,11 +223,11 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value);
 
 int sim_get_stats(const sim_handle* h, sim_stats* out);
 
-/* Synchronises the stream, copies the library's device counters to h_out (HOST, 4 x uint32:
- * [0] scheduling tickets of the last accumulation launch, [1] scatterers whose contributions left the
- * shared-memory tile for global atomics (outside the Doppler window / above the fixed-point range),
- * [2] tile flushes, [3] scatterers whose indices the canonical sequence decided (guard band)) and, when
- * reset != 0, zeroes them. */
+/* Synchronises the stream, copies the library's device counters to h_out (HOST, 4 x uint32) and, when reset != 0,
+ * zeroes them.  [1] scatterers whose contributions left the shared-memory tile for global reductions (outside the
+ * Doppler window / above the fixed-point range / guard band), [3] scatterers whose indices the canonical sequence
+ * decided (guard band); both since the last reset.  [0] and [2] are the accumulation kernel's own scheduling words
+ * (ticket counter, blocks finished): each launch leaves them at 0, they carry no information between launches. */
 int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset);
 
 /* ---- one update without any device allocation by anybody ------------------------------------------ */

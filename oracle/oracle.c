@@ -33,6 +33,9 @@
  * special case, Parseval, brute-force regular-mode sum, an independent numpy restatement); the
  * pulse-pair Doppler mode by tests/test_oracle_pulse_pair.py (the literal arg(C_{i+1} C_i^*) estimator at
  * 50 digits, the analytic f_D plus its closed-form second-order term, aliasing).
+ * The integer decisions of geometry() -- a Doppler coordinate exactly half-way between two bins, a range exactly on
+ * a gate boundary, the edges of the gate window and of the Doppler range -- by tests/test_oracle_decisions.py
+ * (dyadic scenes that land on them without rounding, expected gates and bins as literals).
  * The table gain by tests/test_oracle_lut.py (constant table = isotropic, a table linear in u and v
  * reproduced exactly, a finely sampled Gaussian against the analytic gain within the interpolation bound,
  * mpmath closed form of single scatterers, the frame and the edge rule).

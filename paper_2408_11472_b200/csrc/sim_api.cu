@@ -87,9 +87,9 @@ struct sim_handle {
   // tuning
   int opt_variant, opt_blocks, opt_window, opt_index_path, opt_guard;
   int64_t opt_superchunk;
-  int opt_ncw, opt_stages;          // warps per block; ring depth option (accepted, unused)
+  int opt_ncw;                      // warps per block
   int ws_W, ws_stages, ws_blocks_per_sm;   // planned window width, ring depth, resident blocks per SM
-  int opt_wait_hint, opt_scatter;
+  int opt_scatter;
   int opt_il;
   int opt_pt, opt_epoch;            // scatterers per lane per chunk; scatterers per fixed-point epoch
   size_t smem_per_sm;
@@ -526,8 +526,6 @@ int sim_create(const sim_config* cfg, void* d_workspace, size_t bytes, void* cud
   h->lut_u0 = h->lut_du = h->lut_v0 = h->lut_dv = 0.0;
   h->opt_variant = 4;
   variant_defaults(h);
-  h->opt_stages = 0;
-  h->opt_wait_hint = 0;
   h->opt_scatter = 1;
   h->opt_blocks = 0;
   h->opt_window = 0;
@@ -867,9 +865,6 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
       }
       return SIM_OK;
     }
-    case SIM_OPT_ACC_WAIT_HINT:
-      h->opt_wait_hint = (int)value;
-      return SIM_OK;
     case SIM_OPT_ACC_INTERLEAVE:
       return replan(h->opt_il, (int)value, "interleave not supported by this accumulation variant");
     case SIM_OPT_ACC_SCATTER:
@@ -878,10 +873,6 @@ int sim_set_option(sim_handle* h, int32_t option, int64_t value) {
     case SIM_OPT_ACC_EPOCH:
       if (value < 64 || value > 16383) return fail(h, SIM_ERR_INVALID_ARG, "scatterers per fixed-point epoch: 64..16383");
       h->opt_epoch = (int)value;
-      return SIM_OK;
-    case SIM_OPT_ACC_STAGES:
-      if (value > 8 || value == 1) return fail(h, SIM_ERR_INVALID_ARG, "ring depth: 0 (auto) or 2..8");
-      h->opt_stages = (int)value;   // (accepted for compatibility: the production kernel always uses two stages)
       return SIM_OK;
     case SIM_OPT_GUARD_LSB:
       if (value < 1 || value > (1 << (kFracBits - 2))) return fail(h, SIM_ERR_INVALID_ARG, "guard must be in 1..2^18");
@@ -910,11 +901,6 @@ int sim_read_counters(sim_handle* h, uint32_t* h_out, int32_t reset) {
   if (!h) return fail(nullptr, SIM_ERR_INVALID_ARG, "handle is NULL");
   if (!h_out) return fail(h, SIM_ERR_INVALID_ARG, "h_out is NULL");
   cudaError_t e = cudaMemcpyAsync(h_out, counters(h), 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost, h->stream);
-  if (getenv("SIM_PROFILE")) {
-    unsigned long long pr[5];
-    cudaMemcpy(pr, counters(h) + 8, sizeof(pr), cudaMemcpyDeviceToHost);
-    fprintf(stderr, "PROF wait_full %.3f wait_tile %.3f drain %.3f issue %.3f of total warp-cycles %llu\n", pr[0] / (double)pr[4], pr[1] / (double)pr[4], pr[2] / (double)pr[4], pr[3] / (double)pr[4], pr[4]);
-  }
   if (e == cudaSuccess && reset) e = cudaMemsetAsync(counters(h), 0, kNumCounters * sizeof(uint32_t), h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "read counters");

@@ -8,7 +8,7 @@
 namespace simk {
 
 constexpr int kNumCounters = 64;
-constexpr int kSynMaxPass = 12;                // passes of the mixed-radix inverse FFT (N <= 2048 needs at most 8)
+constexpr int kSynMaxPass = 12;                // passes of the mixed-radix inverse FFT (N <= 4096 needs at most 7: 3^7, 4 * 3^6, 5 * 3^6)
 constexpr int kFracBits = 20;                 // fixed-point fraction bits of the gate / Doppler coordinates
 
 enum Counter : int {

@@ -21,8 +21,8 @@ DOPPLER_ANALYTIC, DOPPLER_PULSE_PAIR = 0, 1
 SYN_FINAL = 1
 GATE_NONE = -(2**31)
 OPT_ACC_VARIANT, OPT_ACC_BLOCKS, OPT_ACC_SUPERCHUNK, OPT_ACC_WINDOW_BINS, OPT_GUARD_LSB, OPT_INDEX_PATH = 1, 2, 3, 4, 5, 6
-OPT_ACC_WARPS, OPT_ACC_STAGES = 9, 10
-OPT_ACC_PER_LANE, OPT_ACC_EPOCH, OPT_ACC_WAIT_HINT, OPT_ACC_SCATTER, OPT_ACC_INTERLEAVE, OPT_ACC_SHAPE = 11, 12, 13, 14, 15, 16
+OPT_ACC_WARPS = 9
+OPT_ACC_PER_LANE, OPT_ACC_EPOCH, OPT_ACC_SCATTER, OPT_ACC_INTERLEAVE, OPT_ACC_SHAPE = 11, 12, 14, 15, 16
 
 EXPORTS = [
     "sim_workspace_bytes", "sim_create", "sim_accumulate_update", "sim_synthesize_pulses",
@@ -274,7 +274,7 @@ class Sim:
     def read_counters(self, reset: bool = False) -> dict:
         a = (C.c_uint32 * 4)()
         self._check(self.lib.sim_read_counters(self._h, a, int(reset)), self._h)
-        return {"tickets": a[0], "escapes": a[1], "flushes": a[2], "index_fallbacks": a[3]}
+        return {"escapes": a[1], "index_fallbacks": a[3]}      # [0], [2]: the kernel's own scheduling words, 0 between launches
 
 
 def accumulate_static(cfg: SimConfig, scat: dict, sat: SimSatState, out: "torch.Tensor | None" = None,
