@@ -55,8 +55,63 @@ def committed_traffic(workload):
     return None
 
 
+class NvmlSampler:
+    """SM clock and throttle reasons of the device, read in-process through NVML every 5 ms DURING the timed region
+    (a timed region of 10 ms is over before `nvidia-smi -lms 100` prints its first line)."""
+    REASONS = ((0x8, "hw_slowdown"), (0x40, "hw_thermal_slowdown"), (0x20, "sw_thermal_slowdown"), (0x4, "sw_power_cap"))
+
+    def __init__(self, dev):
+        import pynvml
+        self.nv = pynvml
+        pynvml.nvmlInit()
+        try:
+            uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+            self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+        except Exception:
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(dev.index or 0)
+        self.mx = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        self.sm, self.mask, self.stop = [], 0, threading.Event()
+
+    def _reasons(self):
+        f = getattr(self.nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or self.nv.nvmlDeviceGetCurrentClocksThrottleReasons
+        return int(f(self.h))
+
+    def _loop(self):
+        while not self.stop.is_set():
+            try:
+                self.sm.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                self.mask |= self._reasons()
+            except Exception:
+                pass
+            self.stop.wait(0.005)
+
+    def __enter__(self):
+        self.t = threading.Thread(target=self._loop, daemon=True)
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=1)
+
+    def summary(self):
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.mx, "reasons": [], "samples": 0, "source": "nvml"}
+        return {"sm_mhz": statistics.median(self.sm), "sm_min_mhz": min(self.sm), "sm_max_mhz": self.mx,
+                "reasons": sorted(n for b, n in self.REASONS if self.mask & b), "samples": len(self.sm),
+                "source": "nvml, 5 ms period, in-process"}
+
+
+def clock_sampler(dev):
+    try:
+        return NvmlSampler(dev)
+    except Exception:
+        return ClockSampler(dev.index or 0)
+
+
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    """Fallback when NVML cannot be loaded: nvidia-smi clocks and throttle reasons DURING the timed region
+    (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -103,7 +158,7 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "samples": len(sm), "source": "nvidia-smi -lms 100"}
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -226,13 +281,28 @@ def empty_launch_us(dev, reps=200):
     return 1e3 * e0.elapsed_time(e1) / reps
 
 
-def timed_run(S, wl, scat, dev, local_rank, steps, warmup, world, dist, opts, peak):
+def scene_copies(scat):
+    """Identical device copies of a scene that successive updates cycle through, so that no update finds part of its
+    input in the 126 MB L2 from the update before: three copies when the scene is below 4 GB (>= 1.4 GB in rotation),
+    the scene itself when it is larger (7.5 GB per pass: nothing survives)."""
+    nbytes = sum(v.numel() * v.element_size() for v in scat.values())
+    if nbytes >= 4e9 or nbytes == 0:
+        return [scat]
+    return [scat] + [{k: v.clone() for k, v in scat.items()} for _ in range(2)]
+
+
+def timed_run(S, wl, scats, dev, local_rank, steps, warmup, world, dist, opts, peak, doppler_mode=0, lut=None):
     """warmup + steps passes of the whole hot path over device-resident input, timed on the device.
+    scats: identical copies of the (local) scene, used in rotation (scene_copies).
     Returns a dict of measurements (times are the max over ranks)."""
     U, P, G, N = wl.n_updates, wl.pulses_per_update, wl.n_gates, wl.n_doppler
+    scat = scats[0]
     n_local = scat["x"].numel()
     sats = [S.sat_for(wl, u) for u in range(U)]
-    sim = S.Sim(S.config_for(wl, max_pending_updates=U + 1, device=local_rank))
+    sim = S.Sim(S.config_for(wl, max_pending_updates=U + 1, device=local_rank, doppler_mode=doppler_mode))
+    if lut is not None:
+        sim.set_antenna_lut(*lut)
+    turn = [0]
     for kv in opts:
         k, v = kv.split("=")
         sim.set_option(int(k), int(v))
@@ -254,7 +324,8 @@ def timed_run(S, wl, scat, dev, local_rank, steps, warmup, world, dist, opts, pe
             if record and per_update_events:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-            sim.accumulate_update(scat, sats[u])
+            sim.accumulate_update(scats[turn[0] % len(scats)], sats[u])
+            turn[0] += 1
             if record and per_update_events:
                 e1.record(stream)
                 acc_events.append((e0, e1, 1))
@@ -283,7 +354,7 @@ def timed_run(S, wl, scat, dev, local_rank, steps, warmup, world, dist, opts, pe
     sim.read_counters(reset=True)
     launches0 = sim.stats()["kernel_launches"]
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
+    with clock_sampler(dev) as clk:
         barrier()
         ev0.record(stream)
         for _ in range(steps):
@@ -310,6 +381,11 @@ def timed_run(S, wl, scat, dev, local_rank, steps, warmup, world, dist, opts, pe
                      "launch_gaps_per_step": ms_per_step - U * acc_ms_mean - syn_ms_mean},
         "roofline": {"bound": "hbm", "kernel": "acc_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": committed_traffic(wl.name),
+                     "traffic_source": "committed ncu --set full capture of this kernel on this workload "
+                                       "(profiles/acc_kernel_traffic.csv); not measured in this run",
+                     "l2": (f"{len(scats)} identical device copies of the scene used in rotation "
+                            f"({len(scats) * BYTES_PER_SCATTERER * n_local / 1e9:.2f} GB >> 126 MB L2): every update reads from DRAM"
+                            if len(scats) > 1 else "one pass reads more than the L2 holds many times over: no flush needed"),
                      "algorithmic_bytes_per_launch": BYTES_PER_SCATTERER * n_local, "launch_ms": acc_ms_mean,
                      "frac_of_8TBs_nominal": achieved / 8000.0},
         "synthesis": {"kernel": "synth_kernel", "ms": syn_ms_mean, "algorithmic_bytes": syn_bytes,
@@ -319,6 +395,61 @@ def timed_run(S, wl, scat, dev, local_rank, steps, warmup, world, dist, opts, pe
         "index_fallbacks_per_step": counters["index_fallbacks"] / max(1, steps),
         "steps": steps, "warmup": warmup,
     }
+
+
+def next_row(name, what, wl, r):
+    """One SURVEY.md 8(f) row measured like the main line (same events, same clock sampler)."""
+    return {"row": name, "what": what, "workload": wl.name, "ms_per_update": r["split_ms"]["accumulate_per_update"],
+            "value": wl.n_scatterers / (r["split_ms"]["accumulate_per_update"] * 1e-3), "unit": "scatterers/s",
+            "frac_of_hbm_peak": r["roofline"]["frac"], "steps": r["steps"], "clocks": r["clocks"]}
+
+
+def gaussian_table(wl, dev, n=512):
+    """A synthetic u-v antenna table for the timing of the tabulated-gain path: the analytic Gaussian of the workload
+    sampled on n x n points over the directions the scene spans (the paper's tables are not available)."""
+    half = 1.05 * max(wl.n_along, wl.n_cross) * wl.spacing_m / 2.0 / W.ALTITUDE_M
+    step = 2.0 * half / (n - 1)
+    u = -half + step * torch.arange(n, device=dev, dtype=torch.float64)
+    g = torch.exp(-wl.antenna_alpha * (u[None, :] ** 2 + u[:, None] ** 2))
+    return torch.complex(g, torch.zeros_like(g)).to(torch.complex64).contiguous(), -half, step, -half, step
+
+
+def event_ms(dev, fn, reps=5):
+    """Median device time of fn() over reps runs after one untimed run, with the clock sampler around them."""
+    stream = torch.cuda.current_stream(dev)
+    fn()
+    torch.cuda.synchronize(dev)
+    ts = []
+    with clock_sampler(dev) as clk:
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            ts.append(e0.elapsed_time(e1))
+    return statistics.median(ts), clk.summary()
+
+
+def regular_row(S, wl, scat, dev, n_pulses=256):
+    """sim_regular_pulses: every scatterer at every pulse, the scene resident on the device."""
+    sim = S.Sim(S.config_for(wl, device=dev.index or 0))
+    out = torch.empty((n_pulses, wl.n_gates), dtype=torch.complex64, device=dev)
+    ms, clk = event_ms(dev, lambda: sim.regular_pulses(scat, S.sat_for(wl, 0), 0, n_pulses, out=out))
+    return {"row": "regular_mode", "what": f"sim_regular_pulses, {n_pulses} pulses (PAPER.md:27, :33)", "workload": wl.name,
+            "ms": ms, "value": wl.n_scatterers * n_pulses / (ms * 1e-3), "unit": "scatterer-pulses/s", "clocks": clk}
+
+
+def burst_row(S, wl, dev, burst=64):
+    """sim_burst_beams on an IQ stream of the track config's shape (random values)."""
+    sim = S.Sim(S.config_for(wl, device=dev.index or 0))
+    iq = torch.randn((wl.n_pulses, wl.n_gates, 2), device=dev, generator=torch.Generator(device=dev).manual_seed(5))
+    iq = torch.view_as_complex(iq).contiguous()
+    ms, clk = event_ms(dev, lambda: sim.burst_beams(iq, burst), reps=20)
+    nbytes = 2 * iq.numel() * 8
+    return {"row": "burst_fft", "what": f"sim_burst_beams, bursts of {burst} pulses (PAPER.md:145-149)", "workload": wl.name,
+            "ms": ms, "value": iq.numel() / (ms * 1e-3), "unit": "IQ samples/s", "algorithmic_bytes": nbytes,
+            "achieved_gbs": nbytes / (ms * 1e-3) / 1e9, "clocks": clk}
 
 
 OTHER_WORKLOADS = ["nadir_patch_16m", "sweep_p16", "sweep_p32", "sweep_p64", "sweep_p128", "sweep_p256", "sweep_p512",
@@ -344,11 +475,32 @@ def main():
         run_reference(args, wl)
         return
 
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # `python bench.py --gpus N` by itself: start the N ranks here (one process per GPU under torchrun, the same
+        # command line the driver uses), instead of quietly measuring one GPU
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: this node shows {torch.cuda.device_count()} CUDA device(s)")
+        import socket
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")          # the init lines name every rank, its GPU and the transport
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        sys.stdout.flush()
+        os.execve(sys.executable, cmd, env)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    if world != args.gpus and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE = {world}: n_gpus reports the {world} rank(s) that run",
+              file=sys.stderr)
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} has no GPU (LOCAL_RANK {local_rank}, {torch.cuda.device_count()} visible)")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     dist = None
@@ -375,8 +527,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    main_run = timed_run(S, wl, scat, dev, local_rank, args.steps, args.warmup, world, dist, args.opt, peak)
+    scats = scene_copies(scat)
+    main_run = timed_run(S, wl, scats, dev, local_rank, args.steps, args.warmup, world, dist, args.opt, peak)
     main_run["roofline"]["peak_source"] = peak_src
+    del scats[1:]
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -435,6 +589,18 @@ def main():
                         "single_thread_value": v1, "sample_in_window_fraction": inw,
                         "scene_in_window_fraction_update0": main_run["in_window_fraction_update0"]}
 
+    # ---- SURVEY.md 8(f) rows on this box: pulse-pair Doppler and the tabulated gain on this workload ----
+    next_rows = []
+    if world == 1 and not args.no_others:
+        k_next = max(3, min(args.steps, 5))
+        r = timed_run(S, wl, [scat], dev, local_rank, k_next, 3, 1, None, args.opt, peak, doppler_mode=S.DOPPLER_PULSE_PAIR)
+        next_rows.append(next_row("pulse_pair_doppler", "sim_accumulate_update, SIM_DOPPLER_PULSE_PAIR (PAPER.md:81-83)", wl, r))
+        tab = gaussian_table(wl, dev)
+        r = timed_run(S, wl, [scat], dev, local_rank, k_next, 3, 1, None, args.opt, peak, lut=tab)
+        next_rows.append(next_row("tabulated_antenna_gain", "sim_accumulate_update after sim_set_antenna_lut, 512 x 512 "
+                                  "complex u-v table (PAPER.md:35)", wl, r))
+        del tab
+
     # ---- the other configs, short runs with the same event timing (configs[1], [3], [4]) ----
     others = []
     if world == 1 and not args.no_others and args.workload == DEFAULT_WORKLOAD:
@@ -448,10 +614,15 @@ def main():
                 scenes.clear()
                 torch.cuda.empty_cache()
                 scenes[key] = W.scatterers(w2, device=dev)
+                scenes[key] = scene_copies(scenes[key])
             r = timed_run(S, w2, scenes[key], dev, local_rank, 3 if w2.n_updates > 16 else 10, 3, 1, None, args.opt, peak)
             others.append({"workload": name, "scatterers": w2.n_scatterers, "gates": w2.n_gates, "doppler_bins": w2.n_doppler,
                            "pulses_per_update": w2.pulses_per_update, "updates": w2.n_updates, **r})
+            if name == "nadir_patch_16m":     # regular mode on the same resident scene
+                next_rows.append(regular_row(S, w2, scenes[key][0], dev))
         scenes.clear()
+        torch.cuda.empty_cache()
+        next_rows.append(burst_row(S, W.get("track_segment_67m"), dev))
 
     if rank == 0:
         out = {
@@ -463,8 +634,7 @@ def main():
             "dtype": "f32", "dtype_note": "fp32 amplitudes, accumulation (block-floating int32 tiles, fp64 global accumulator) and FFT; fp64 range, gate/bin index and phase reduction",
             "data": "synthetic",
             "config": {"workload": wl.name, "scatterers": wl.n_scatterers, "gates": G, "doppler_bins": N,
-                       "pulses_per_update": P, "updates": U, "l2": "inputs larger than L2 (no flush needed)"
-                       if BYTES_PER_SCATTERER * n_local > 2.5e8 else "inputs fit L2: not a bench workload",
+                       "pulses_per_update": P, "updates": U, "l2": main_run["roofline"]["l2"],
                        "parallelism": f"scatterer-sharded x{world}, all-reduce of spectra" if world > 1 else "1 GPU",
                        "in_window_fraction_update0": main_run["in_window_fraction_update0"]},
             "iq_samples_per_s": main_run["iq_samples_per_s"],
@@ -474,7 +644,7 @@ def main():
             "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": main_run["gpu_launches"],
             "clocks": main_run["clocks"], "escapes_per_step": main_run["escapes_per_step"],
             "index_fallbacks_per_step": main_run["index_fallbacks_per_step"],
-            "other_workloads": others,
+            "other_workloads": others, "next_rows": next_rows,
         }
         print(json.dumps(out), flush=True)
     if world > 1:
