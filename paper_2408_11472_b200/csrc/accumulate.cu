@@ -128,11 +128,6 @@ __device__ __forceinline__ void stream_open(const UnitTable& ut, ChunkStream& s)
   ++s.unit;
 }
 
-// round(a * b) for |a b| <= 2^22 by the 1.5 * 2^23 trick (round to nearest even: unbiased), as an int
-__device__ __forceinline__ int fx_round(float a, float b) {
-  return __float_as_int(fmaf(a, b, 12582912.0f)) - 0x4B400000;
-}
-
 template <int PT>
 struct Vec;
 template <>

@@ -1,4 +1,4 @@
-// Shared-memory, mbarrier and TMA bulk-copy primitives (inline PTX, sm_100a).  32-bit shared-window
+// Shared-memory, mbarrier and asynchronous-copy primitives (inline PTX, sm_100a).  32-bit shared-window
 // addresses throughout: computed once with addr(), then plain integer arithmetic.
 #pragma once
 #include <cuda_runtime.h>
@@ -11,12 +11,6 @@ __device__ __forceinline__ unsigned addr(const void* ptr) { return (unsigned)__c
 __device__ __forceinline__ void red_add(unsigned a, int v) {
   asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
-__device__ __forceinline__ void red_min(unsigned a, int v) {
-  asm volatile("red.shared.min.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-__device__ __forceinline__ void red_max(unsigned a, int v) {
-  asm volatile("red.shared.max.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
 __device__ __forceinline__ int cas(unsigned a, int cmp, int val) {
   int old;
   asm volatile("atom.shared.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(a), "r"(cmp), "r"(val) : "memory");
@@ -27,21 +21,6 @@ __device__ __forceinline__ int atom_add_acq_rel(unsigned a, int v) {
   int old;
   asm volatile("atom.acq_rel.cta.shared.add.s32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(v) : "memory");
   return old;
-}
-__device__ __forceinline__ int cas_acquire(unsigned a, int cmp, int val) {
-  int old;
-  asm volatile("atom.acquire.cta.shared.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(a), "r"(cmp), "r"(val) : "memory");
-  return old;
-}
-// orders this thread's earlier generic-proxy accesses to shared memory before its later async-proxy (bulk copy) ones
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ int4 ld4(unsigned a) {
-  int4 v;
-  asm volatile("ld.shared.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st4(unsigned a, int4 v) {
-  asm volatile("st.shared.v4.s32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ int2 ld2(unsigned a) {
   int2 v;
@@ -88,9 +67,6 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
 __device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 // Blocks until the phase of parity `parity` has completed (acquire at CTA scope).
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
@@ -145,18 +121,10 @@ __device__ __forceinline__ float4 ldf4(unsigned a) {
 __device__ __forceinline__ void cp_async16(unsigned dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void* src) { asm volatile("prefetch.global.L2 [%0];" ::"l"(src)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
-// ---- TMA bulk copy global -> shared, completion counted in bytes on the mbarrier ----
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-               "l"(src), "r"(bytes), "r"(bar)
-               : "memory");
-}
-
 }  // namespace sh
 }  // namespace simk

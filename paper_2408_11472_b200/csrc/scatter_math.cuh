@@ -117,43 +117,7 @@ __device__ __forceinline__ Pre pre_part(const AccParams& p, float xf, float yf, 
   return q;
 }
 
-// The polynomial index path WITHOUT the guard-band call: fills `o` and sets `near` when a coordinate lies in the
-// guard band (the caller then lets the canonical sequence decide; until then `o` is not trustworthy).
-// MODE = kIdxFast or kIdxFastPulsePair.  Returns `live`.
-template <int MODE>
-__device__ __forceinline__ bool index_fast(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
-                                           bool live, Idx& o, bool& near) {
-  const double u = q.u;
-  const double gf = u * fma(u, fma(u, p.g3, p.g2), p.g1);
-  const int gfx = __double2loint(__dadd_rd(gf, kMagicFx));            // floor(gf * 2^20)
-  const int gfrac = gfx & (kFxOne - 1);
-  const double dvx = (double)vxf - p.svx, dvy = (double)vyf - p.svy, dvz = (double)vzf - p.svz;
-  const double num = fma(dvz, q.dz, fma(dvy, q.dy, dvx * q.dx));
-  double kf;
-  if (MODE == kIdxFastPulsePair) {
-    // R' - R = w / (R' + R) with w = R'^2 - R^2 = (2 num + |dv|^2 / PRF) / PRF, computed without cancellation, and
-    // R' + R = 2 rg0 + 2 (R - rg0) + (R' - R);  1 / (1 + e) = 1 - e + e^2 (e <= 1e-4)
-    const double dv2 = fma(dvz, dvz, fma(dvy, dvy, dvx * dvx));
-    const double w = p.pri * fma(dv2, p.pri, num + num);
-    const double e = fma(w, p.inv_2rg0, gf * p.two_dR) * p.inv_2rg0;
-    kf = (w * p.cP_2rg0) * fma(e, e - 1.0, 1.0);
-  } else {
-    kf = num * fma(u, fma(u, p.j2, p.j1), p.j0);
-  }
-  const int kfx = __double2loint(__dadd_rd(kf, kMagicFxHalf));        // floor((kf + 0.5) * 2^20)
-  const int kfrac = kfx & (kFxOne - 1);
-  const int gk = MODE == kIdxFastPulsePair ? p.guard_k : p.guard;   // pulse-pair: wider Doppler guard band
-  const unsigned span = (unsigned)(kFxOne - 2 * p.guard), span_k = (unsigned)(kFxOne - 2 * gk);
-  near = live && (((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) | !(fabs(kf) < 1024.0));
-  o.g0 = gfx >> kFracBits;
-  o.k = kfx >> kFracBits;
-  o.w1 = (float)gfrac * p.w_scale;
-  o.fr = cycles_fraction(fma(gf, p.cq, p.fr0));
-  o.gfx = (float)gfx;
-  return live;
-}
-
-// The same polynomial path in the form the production kernel keeps alive across the amplitude code: the two fixed-point
+// The polynomial index path (MODE = kIdxFast or kIdxFastPulsePair) in the form the production kernel keeps alive across the amplitude code: the two fixed-point
 // coordinates and the phase; gate, bin, weight and the guard-band test are derived from them afterwards.
 struct Fx {
   int gfx;     // floor(gf * 2^kFracBits)
@@ -201,20 +165,6 @@ __device__ __forceinline__ bool fx_near(const AccParams& p, const Fx& f) {
   const unsigned span = (unsigned)(kFxOne - 2 * p.guard), span_k = (unsigned)(kFxOne - 2 * gk);
   const int gfrac = f.gfx & (kFxOne - 1), kfrac = f.kfx & (kFxOne - 1);
   return ((unsigned)(gfrac - p.guard) >= span) | ((unsigned)(kfrac - gk) >= span_k) | (f.kfx == INT_MIN);
-}
-
-// Gate, bin, weight, phase.  Returns true when the scatterer lands in the window.
-template <int MODE>
-__device__ __forceinline__ bool index_part(const AccParams& p, const Pre& q, float vxf, float vyf, float vzf,
-                                           bool live, Idx& o, unsigned& fallbacks) {
-  if (MODE == kIdxCanonical) return live && canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
-  bool near;
-  live = index_fast<MODE>(p, q, vxf, vyf, vzf, live, o, near);
-  if (near) {  // rare: a coordinate sits in the guard band
-    ++fallbacks;
-    return canonical(p, q.dx, q.dy, q.dz, vxf, vyf, vzf, o);
-  }
-  return live;
 }
 
 __device__ __forceinline__ float sqrt_approx(float v) {
