@@ -239,9 +239,25 @@ cudaError_t plan_ws(sim_handle* h) {
   if (budget > h->smem_optin - 4096) budget = h->smem_optin - 4096;   // the kernels' static shared memory (< 3 KB) counts against the opt-in limit
   const size_t stage = smem(0, 0, 1) - smem(0, 0, 0);
   const int st = 2;   // every lane copies one chunk ahead of its reads: two stages
-  int w = h->opt_window > 0 ? h->opt_window : 20;
-  if (w > N) w = N;
-  while (w > 1 && smem(G, w, 0) + st * stage > budget) --w;
+  int want = h->opt_window > 0 ? h->opt_window : 20;
+  if (want > N) want = N;
+  auto widest = [&](size_t bytes) {
+    int v = want;
+    while (v > 1 && smem(G, v, 0) + st * stage > bytes) --v;
+    return v;
+  };
+  int w = widest(budget);
+  if (target == 2 && w < 4 && want >= 4) {
+    // Very many gates (beyond ~440): two blocks per SM leave no room for even a 4-bin window, and every contribution
+    // would go to the global fp64 reductions (measured on the 16.8M patch, G = 512 / 1024: 621 / 470 us per update).
+    // One block per SM with all of the SM's shared memory holds a window again (166 / 175 us).  A 4-bin window at two
+    // blocks per SM, where it fits (G = 192, 256: 117 us), beats a 20-bin window at one block (174-179 us), so the
+    // re-plan is taken only when the two-block plan has no window at all.
+    size_t one = h->smem_per_sm > 2048 ? h->smem_per_sm - 2048 : 0;
+    if (one > h->smem_optin - 4096) one = h->smem_optin - 4096;
+    const int w1 = widest(one);
+    if (w1 > w) w = w1;
+  }
   if (h->opt_window == 0 && acc_row_stride(w) <= N) w = acc_row_stride(w);   // the padding columns of a row are free
   h->ws_W = w;
   h->ws_stages = st;
