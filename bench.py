@@ -247,7 +247,9 @@ def run_reference(args, wl):
         "ms_per_step": 1e3 * statistics.mean(step_s), "ms_per_full_step_extrapolated": 1e3 * wl.n_updates * wl.n_scatterers / value,
         "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wl.name, "note": "oracle on host cores; each step is a bounded sample of this workload "
+        "config": {"workload": wl.name, "scatterers": wl.n_scatterers, "gates": wl.n_gates, "doppler_bins": wl.n_doppler,
+                   "pulses_per_update": wl.pulses_per_update, "updates": wl.n_updates,
+                   "note": "oracle on host cores; each step is a bounded sample of this workload "
                    f"(same recipe, {scat['x'].numel()} scatterers as whole rows spread evenly over the scene); "
                    "ms_per_step is the measured time of a sampled step, value the rate extrapolated to whole steps"},
         "cpu_baseline": {"value": value, "unit": "scatterers/s", "cores": nthreads, "kind": "oracle",
